@@ -1,0 +1,152 @@
+/*
+ * mttkrp.h - C-ABI of libmttkrp_b200: all-mode sparse MTTKRP with dynamic tensor remapping
+ * on one NVIDIA B200 (sm_100a).
+ *
+ * The operation (arxiv 2405.08470; citations are PAPER.md line numbers):
+ *   Y_d[i_d, r] = sum over nonzeros k of val_k * prod_{m != d} A_m[i_m(k), r]
+ *     - Eq. 1 and the elementwise form of Sec. 2.1.5;
+ *     - Alg. 2 "Elementwise Computation for mode d";
+ *     - Alg. 3 "Dynamic Tensor Remapping": before mode d the nonzeros are
+ *       re-ordered into the mode-d layout, in which all nonzeros of one output row are adjacent
+ *       (Observation 2) and every element has a unique position
+ *       (Observation 1);
+ *     - Alg. 5: for d = 0..N-1 { compute mode d; barrier; swap(T_in, T_out) }.
+ *
+ * Conventions (all entry points):
+ *   - Every call returns a status; nothing throws, aborts or prints.  mttkrp_last_error() gives a
+ *     thread-local message for the last non-OK status.
+ *   - "device" pointers are CUDA device memory of the current device, "host" pointers are ordinary
+ *     host memory.  Device pointers must be 16-byte aligned.
+ *   - The library never allocates device memory: the caller passes one workspace (size from
+ *     mttkrp_workspace_bytes) which the handle borrows until mttkrp_destroy.
+ *   - cuda_stream is a cudaStream_t passed as void* (NULL = default stream).  mttkrp_mode and
+ *     mttkrp_sweep are asynchronous on that stream; mttkrp_create synchronises the stream because
+ *     it reads back counts and the index-error flag.
+ *   - Indices are 0-based.  Duplicate coordinates are legal and add.  nnz == 0 is legal.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns MTTKRP_ECUDA.
+ *   - A handle is not thread-safe; distinct handles are independent.
+ */
+#ifndef MTTKRP_B200_H
+#define MTTKRP_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MTTKRP_MAX_MODES 8
+
+typedef struct mttkrp_handle_s* mttkrp_handle_t; /* opaque host object */
+
+typedef enum {
+    MTTKRP_OK = 0,
+    MTTKRP_EINVAL = 1,       /* bad argument (null pointer, size, mode, rank, alignment) */
+    MTTKRP_EINDEX = 2,       /* an index is outside [0, dims[m]) (detected on the device in create) */
+    MTTKRP_EUNSUPPORTED = 3, /* nmodes outside [2,8], R not in {8,16,32,64}, nnz >= 2^31 */
+    MTTKRP_EWORKSPACE = 4,   /* workspace too small or misaligned */
+    MTTKRP_ECUDA = 5         /* a CUDA runtime call or kernel launch failed */
+} mttkrp_status_t;
+
+/* What a handle holds; filled by mttkrp_get_info (host struct). */
+typedef struct {
+    int32_t nmodes;
+    int32_t cur_layout;                  /* mode whose order the resident tensor copy is in (0 after create) */
+    int64_t nnz;
+    int64_t dims[MTTKRP_MAX_MODES];
+    int32_t record_bytes;                /* bytes per nonzero in the device format: 4*(nmodes+1) */
+    int32_t shard_nnz;                   /* nonzeros per thread-block shard */
+    int64_t num_shards;                  /* ceil(nnz / shard_nnz); same for every mode */
+    int64_t num_split_rows[MTTKRP_MAX_MODES];  /* output rows whose nonzeros span more than one shard */
+    int64_t num_empty_rows[MTTKRP_MAX_MODES];  /* output rows with no nonzero (stored as zeros) */
+    int64_t bytes_held;                  /* device bytes the handle keeps after create (both tensor copies, maps, tables) */
+    int64_t bytes_paper_format;          /* FLYCOO bytes by the paper's formula, PAPER.md:187:
+                                            nnz * (N*ceil(log2 nnz) + sum ceil(log2 I_h) + 32) / 8 */
+    int64_t remaps_done;                 /* remap passes executed since create */
+    int32_t key_order[MTTKRP_MAX_MODES][MTTKRP_MAX_MODES];
+                                         /* key_order[d] = sort-key order of the mode-d layout:
+                                            key_order[d][0] == d, then the other modes (major to minor) */
+} mttkrp_info_t;
+
+/*
+ * Device workspace the handle needs for a tensor of this shape (pure host arithmetic).
+ * max_rank: largest R that will be used with the *_host entry points (staging for factors and
+ * output is then included); pass 0 if only device-pointer entry points are used.
+ */
+mttkrp_status_t mttkrp_workspace_bytes(int nmodes, const int64_t* dims /*host*/, int64_t nnz,
+                                       int max_rank, size_t* bytes /*host, out*/);
+
+/*
+ * Build the device format from COO (Sec. 3.2/3.5 PAPER.md:147-149,183-189 as behaviour; the
+ * layout itself is this library's): for every mode d a stable sort of the nonzeros by the key
+ * tuple key_order[d] (output index first), the position maps between consecutive layouts (the
+ * paper's remap ids), the empty-row and split-row tables, and the tensor copy in
+ * mode-0 order (Alg. 5 input PAPER.md:308).
+ *
+ *   idx   device int32 [nmodes][nnz] (SoA, idx[m*nnz + k]), vals device fp32 [nnz], dims host.
+ *   The COO arrays are only read, and are no longer needed once the call returns.
+ *   workspace: device, >= mttkrp_workspace_bytes(...), borrowed until destroy.
+ * Errors: EINVAL / EUNSUPPORTED / EWORKSPACE before any launch; EINDEX if an index is out of
+ * range; ECUDA.  On error *out is NULL and the workspace contents are undefined.
+ */
+mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* dims, int64_t nnz,
+                              const int32_t* idx, const float* vals, int max_rank,
+                              void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * Y_d = MTTKRP along mode d (Alg. 2 + Alg. 3 + one iteration of Alg. 5's loop).
+ *   factors: host array of nmodes device pointers; A_m is fp32 [dims[m]][R] row-major (ld = R).
+ *            factors[d] is not read and may be NULL.
+ *   out:     device fp32 [dims[d]][R] row-major; fully overwritten (rows without nonzeros get 0).
+ *            Must not alias a factor that is read.
+ *   Any d in any order.  If the resident layout is not d the tensor is first remapped
+ *   (cur -> cur+1 -> ... -> d, one scatter pass per step; the cyclic order of Alg. 5 costs one).
+ */
+mttkrp_status_t mttkrp_mode(mttkrp_handle_t h, int d, const float* const* factors, int R,
+                            float* out, void* cuda_stream);
+
+/* All modes d = 0..nmodes-1 in order (Alg. 5).  outs: host array of nmodes
+ * device pointers, outs[d] as `out` above.  Factors are not updated between modes. */
+mttkrp_status_t mttkrp_sweep(mttkrp_handle_t h, const float* const* factors, int R,
+                             float* const* outs, void* cuda_stream);
+
+/* Only the remap pass into layout d (Alg. 3), no computation; used to time the two separately
+ * and by tests. */
+mttkrp_status_t mttkrp_remap_to(mttkrp_handle_t h, int d, void* cuda_stream);
+
+/*
+ * Same as mttkrp_sweep with HOST buffers: factors[m] host fp32 [dims[m]][R] (pinned memory makes
+ * the copies asynchronous), outs[d] host fp32 [dims[d]][R].  Copies every factor to the
+ * workspace staging area, runs all modes, copies every Y_d back, and synchronises the stream
+ * before returning.  Needs max_rank >= R at create.
+ */
+mttkrp_status_t mttkrp_sweep_host(mttkrp_handle_t h, const float* const* factors, int R,
+                                  float* const* outs, void* cuda_stream);
+
+/* Frees the host object.  Touches no device memory; the workspace is the caller's again. */
+mttkrp_status_t mttkrp_destroy(mttkrp_handle_t h);
+
+/* Thread-local message of the last failing call ("" if none). */
+const char* mttkrp_last_error(void);
+
+/* Introspection for tests and reports. */
+mttkrp_status_t mttkrp_get_info(mttkrp_handle_t h, mttkrp_info_t* info /*host, out*/);
+
+/* perm_dev[k] (device uint32 [nnz]) = original COO position of the nonzero at position k of the
+ * mode-d layout, i.e. the stable sort permutation for key_order[d] (Observation 1).
+ * scratch_dev: device uint32 [nnz], clobbered.  Asynchronous on cuda_stream. */
+mttkrp_status_t mttkrp_get_perm(mttkrp_handle_t h, int d, uint32_t* perm_dev, uint32_t* scratch_dev,
+                                void* cuda_stream);
+
+/* Copy the resident tensor copy out as SoA COO in its current layout order (device int32
+ * [nmodes][nnz] in ORIGINAL mode numbering, device fp32 [nnz]).  Test hook for the remap. */
+mttkrp_status_t mttkrp_export_coo(mttkrp_handle_t h, int32_t* idx_dev, float* vals_dev, void* cuda_stream);
+
+/* Library / build identification, e.g. "mttkrp_b200 0.1 sm_100a". */
+const char* mttkrp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MTTKRP_B200_H */

@@ -1,0 +1,236 @@
+// C-ABI of libmttkrp_b200 (include/mttkrp.h): argument checks, the layout state machine
+// (Alg. 5) and the host-buffer convenience entry point.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include "common.cuh"
+
+namespace mk {
+
+static thread_local char g_err[512] = "";
+
+void set_error(const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+void choose_key_order(int N, const int64_t* dims, int d, int* order);   // build.cu
+
+static mttkrp_status_t check_shape(int nmodes, const int64_t* dims, int64_t nnz) {
+    if (!dims) { set_error("dims is NULL"); return MTTKRP_EINVAL; }
+    if (nmodes < 2 || nmodes > kMaxModes) { set_error("nmodes %d outside [2,%d]", nmodes, kMaxModes); return MTTKRP_EUNSUPPORTED; }
+    for (int m = 0; m < nmodes; ++m) {
+        if (dims[m] <= 0) { set_error("dims[%d] = %lld must be positive", m, (long long)dims[m]); return MTTKRP_EINVAL; }
+        if (dims[m] > 0x7fffffffLL) { set_error("dims[%d] exceeds int32", m); return MTTKRP_EUNSUPPORTED; }
+    }
+    if (nnz < 0) { set_error("nnz < 0"); return MTTKRP_EINVAL; }
+    if (nnz >= 0x7fffffffLL) { set_error("nnz >= 2^31 unsupported"); return MTTKRP_EUNSUPPORTED; }
+    return MTTKRP_OK;
+}
+
+static bool valid_rank(int R) { return R == 8 || R == 16 || R == 32 || R == 64; }
+static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+static int ceil_log2(int64_t x) {
+    int b = 0;
+    while (((int64_t)1 << b) < x) ++b;
+    return b;
+}
+
+static mttkrp_status_t ensure_layout(mttkrp_handle_s* h, int d, cudaStream_t st) {
+    while (h->cur != d) MK_TRY(launch_remap(h, h->cur, st));
+    return MTTKRP_OK;
+}
+
+}  // namespace mk
+
+using namespace mk;
+
+extern "C" {
+
+const char* mttkrp_last_error(void) { return g_err; }
+const char* mttkrp_version(void) { return "mttkrp_b200 0.1 sm_100a"; }
+
+mttkrp_status_t mttkrp_workspace_bytes(int nmodes, const int64_t* dims, int64_t nnz, int max_rank, size_t* bytes) {
+    if (!bytes) { set_error("bytes is NULL"); return MTTKRP_EINVAL; }
+    MK_TRY(check_shape(nmodes, dims, nnz));
+    if (max_rank != 0 && !valid_rank(max_rank)) { set_error("max_rank %d not in {0,8,16,32,64}", max_rank); return MTTKRP_EUNSUPPORTED; }
+    WorkspacePlan p;
+    MK_TRY(plan_workspace(nmodes, dims, nnz, max_rank, &p));
+    *bytes = p.total;
+    return MTTKRP_OK;
+}
+
+mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* dims, int64_t nnz, const int32_t* idx,
+                              const float* vals, int max_rank, void* workspace, size_t workspace_bytes,
+                              void* cuda_stream) {
+    if (!out) { set_error("out is NULL"); return MTTKRP_EINVAL; }
+    *out = nullptr;
+    MK_TRY(check_shape(nmodes, dims, nnz));
+    if (max_rank != 0 && !valid_rank(max_rank)) { set_error("max_rank %d not in {0,8,16,32,64}", max_rank); return MTTKRP_EUNSUPPORTED; }
+    if (nnz > 0 && (!idx || !vals)) { set_error("idx/vals is NULL"); return MTTKRP_EINVAL; }
+    if (!workspace) { set_error("workspace is NULL"); return MTTKRP_EWORKSPACE; }
+    if (reinterpret_cast<uintptr_t>(workspace) & 255u) { set_error("workspace must be 256-byte aligned"); return MTTKRP_EWORKSPACE; }
+    if (nnz > 0 && (!aligned16(idx) || !aligned16(vals))) { set_error("idx/vals must be 16-byte aligned"); return MTTKRP_EINVAL; }
+    WorkspacePlan p;
+    MK_TRY(plan_workspace(nmodes, dims, nnz, max_rank, &p));
+    if (workspace_bytes < p.total) {
+        set_error("workspace %zu bytes < required %zu", workspace_bytes, p.total);
+        return MTTKRP_EWORKSPACE;
+    }
+    int dev = 0;
+    MK_CUDA(cudaGetDevice(&dev));
+
+    mttkrp_handle_s* h = new (std::nothrow) mttkrp_handle_s();
+    if (!h) { set_error("out of host memory"); return MTTKRP_EINVAL; }
+    memset(h, 0, sizeof(*h));
+    char* ws = static_cast<char*>(workspace);
+    h->N = nmodes;
+    h->nnz = nnz;
+    for (int m = 0; m < nmodes; ++m) h->dims[m] = dims[m];
+    h->rec_words = nmodes + 1;
+    h->shard_nnz = p.shard_nnz;
+    h->num_shards = p.num_shards;
+    h->rec_cur = reinterpret_cast<uint32_t*>(ws + p.rec_a);
+    h->rec_alt = reinterpret_cast<uint32_t*>(ws + p.rec_b);
+    h->perm0 = reinterpret_cast<uint32_t*>(ws + p.perm0);
+    h->carry = reinterpret_cast<float*>(ws + p.carry);
+    h->cur = 0;
+    h->max_rank = max_rank;
+    h->device = dev;
+    for (int d = 0; d < nmodes; ++d) {
+        ModeMeta& mm = h->mode[d];
+        choose_key_order(nmodes, dims, d, mm.order);
+        for (int l = 0; l < nmodes; ++l) mm.pos[mm.order[l]] = l;
+        mm.next = reinterpret_cast<uint32_t*>(ws + p.next[d]);
+        mm.empty_rows = reinterpret_cast<uint32_t*>(ws + p.empty[d]);
+        mm.chains = reinterpret_cast<uint32_t*>(ws + p.chains[d]);
+        if (max_rank > 0) {
+            h->stage_fac[d] = reinterpret_cast<float*>(ws + p.stage_fac[d]);
+            h->stage_out[d] = reinterpret_cast<float*>(ws + p.stage_out[d]);
+        }
+    }
+    h->bytes_held = (int64_t)(p.persistent_end + (size_t)(nmodes + 1) * 4 * (size_t)nnz);
+    mttkrp_status_t s = build_format(h, p, ws, idx, vals, static_cast<cudaStream_t>(cuda_stream));
+    if (s != MTTKRP_OK) { delete h; return s; }
+    *out = h;
+    return MTTKRP_OK;
+}
+
+static mttkrp_status_t check_mode_args(mttkrp_handle_t h, int d, const float* const* factors, int R, const float* out) {
+    if (!h) { set_error("handle is NULL"); return MTTKRP_EINVAL; }
+    if (d < 0 || d >= h->N) { set_error("mode %d outside [0,%d)", d, h->N); return MTTKRP_EINVAL; }
+    if (!valid_rank(R)) { set_error("unsupported rank %d (8, 16, 32, 64)", R); return MTTKRP_EUNSUPPORTED; }
+    if (!factors || !out) { set_error("factors/out is NULL"); return MTTKRP_EINVAL; }
+    if (!aligned16(out)) { set_error("out must be 16-byte aligned"); return MTTKRP_EINVAL; }
+    for (int m = 0; m < h->N; ++m) {
+        if (m == d) continue;
+        if (!factors[m]) { set_error("factors[%d] is NULL", m); return MTTKRP_EINVAL; }
+        if (!aligned16(factors[m])) { set_error("factors[%d] must be 16-byte aligned", m); return MTTKRP_EINVAL; }
+        if (factors[m] == out) { set_error("out aliases factors[%d]", m); return MTTKRP_EINVAL; }
+    }
+    return MTTKRP_OK;
+}
+
+mttkrp_status_t mttkrp_mode(mttkrp_handle_t h, int d, const float* const* factors, int R, float* out, void* cuda_stream) {
+    MK_TRY(check_mode_args(h, d, factors, R, out));
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    MK_TRY(ensure_layout(h, d, st));
+    return launch_mttkrp(h, d, factors, R, out, st);
+}
+
+mttkrp_status_t mttkrp_sweep(mttkrp_handle_t h, const float* const* factors, int R, float* const* outs, void* cuda_stream) {
+    if (!h) { set_error("handle is NULL"); return MTTKRP_EINVAL; }
+    if (!outs) { set_error("outs is NULL"); return MTTKRP_EINVAL; }
+    for (int d = 0; d < h->N; ++d) MK_TRY(check_mode_args(h, d, factors, R, outs[d]));
+    for (int d = 0; d < h->N; ++d) MK_TRY(mttkrp_mode(h, d, factors, R, outs[d], cuda_stream));
+    return MTTKRP_OK;
+}
+
+mttkrp_status_t mttkrp_remap_to(mttkrp_handle_t h, int d, void* cuda_stream) {
+    if (!h) { set_error("handle is NULL"); return MTTKRP_EINVAL; }
+    if (d < 0 || d >= h->N) { set_error("mode %d outside [0,%d)", d, h->N); return MTTKRP_EINVAL; }
+    return ensure_layout(h, d, static_cast<cudaStream_t>(cuda_stream));
+}
+
+mttkrp_status_t mttkrp_sweep_host(mttkrp_handle_t h, const float* const* factors, int R, float* const* outs,
+                                  void* cuda_stream) {
+    if (!h) { set_error("handle is NULL"); return MTTKRP_EINVAL; }
+    if (!valid_rank(R)) { set_error("unsupported rank %d (8, 16, 32, 64)", R); return MTTKRP_EUNSUPPORTED; }
+    if (R > h->max_rank) { set_error("R %d > max_rank %d given at create", R, h->max_rank); return MTTKRP_EINVAL; }
+    if (!factors || !outs) { set_error("factors/outs is NULL"); return MTTKRP_EINVAL; }
+    for (int m = 0; m < h->N; ++m)
+        if (!factors[m] || !outs[m]) { set_error("factors[%d]/outs[%d] is NULL", m, m); return MTTKRP_EINVAL; }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const float* dfac[kMaxModes];
+    for (int m = 0; m < h->N; ++m) {
+        MK_CUDA(cudaMemcpyAsync(h->stage_fac[m], factors[m], (size_t)h->dims[m] * R * 4, cudaMemcpyHostToDevice, st));
+        dfac[m] = h->stage_fac[m];
+    }
+    for (int d = 0; d < h->N; ++d) {
+        MK_TRY(ensure_layout(h, d, st));
+        MK_TRY(launch_mttkrp(h, d, dfac, R, h->stage_out[d], st));
+        MK_CUDA(cudaMemcpyAsync(outs[d], h->stage_out[d], (size_t)h->dims[d] * R * 4, cudaMemcpyDeviceToHost, st));
+    }
+    MK_CUDA(cudaStreamSynchronize(st));
+    return MTTKRP_OK;
+}
+
+mttkrp_status_t mttkrp_destroy(mttkrp_handle_t h) {
+    if (!h) { set_error("handle is NULL"); return MTTKRP_EINVAL; }
+    delete h;
+    return MTTKRP_OK;
+}
+
+mttkrp_status_t mttkrp_get_info(mttkrp_handle_t h, mttkrp_info_t* info) {
+    if (!h || !info) { set_error("handle/info is NULL"); return MTTKRP_EINVAL; }
+    memset(info, 0, sizeof(*info));
+    info->nmodes = h->N;
+    info->cur_layout = h->cur;
+    info->nnz = h->nnz;
+    int64_t bits = 32;
+    for (int m = 0; m < h->N; ++m) {
+        info->dims[m] = h->dims[m];
+        info->num_split_rows[m] = h->mode[m].n_chains;
+        info->num_empty_rows[m] = h->mode[m].n_empty;
+        for (int l = 0; l < h->N; ++l) info->key_order[m][l] = h->mode[m].order[l];
+        bits += ceil_log2(h->dims[m]);
+    }
+    bits += (int64_t)h->N * ceil_log2(h->nnz > 1 ? h->nnz : 2);
+    info->record_bytes = 4 * (h->N + 1);
+    info->shard_nnz = h->shard_nnz;
+    info->num_shards = h->num_shards;
+    info->bytes_held = h->bytes_held;
+    info->bytes_paper_format = (h->nnz * bits + 7) / 8;
+    info->remaps_done = h->remaps_done;
+    return MTTKRP_OK;
+}
+
+mttkrp_status_t mttkrp_get_perm(mttkrp_handle_t h, int d, uint32_t* perm_dev, uint32_t* scratch_dev, void* cuda_stream) {
+    if (!h) { set_error("handle is NULL"); return MTTKRP_EINVAL; }
+    if (d < 0 || d >= h->N) { set_error("mode %d outside [0,%d)", d, h->N); return MTTKRP_EINVAL; }
+    if (h->nnz == 0) return MTTKRP_OK;
+    if (!perm_dev || (d > 0 && !scratch_dev)) { set_error("perm/scratch is NULL"); return MTTKRP_EINVAL; }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    // perm_{j+1}[next_j[k]] = perm_j[k]; choose the start buffer so that step d lands in perm_dev.
+    uint32_t* a = (d % 2 == 0) ? perm_dev : scratch_dev;
+    uint32_t* b = (d % 2 == 0) ? scratch_dev : perm_dev;
+    MK_CUDA(cudaMemcpyAsync(a, h->perm0, (size_t)h->nnz * 4, cudaMemcpyDeviceToDevice, st));
+    for (int j = 0; j < d; ++j) {
+        MK_TRY(launch_perm_step(h->mode[j].next, a, b, h->nnz, st));
+        uint32_t* t = a; a = b; b = t;
+    }
+    return MTTKRP_OK;
+}
+
+mttkrp_status_t mttkrp_export_coo(mttkrp_handle_t h, int32_t* idx_dev, float* vals_dev, void* cuda_stream) {
+    if (!h) { set_error("handle is NULL"); return MTTKRP_EINVAL; }
+    if (h->nnz == 0) return MTTKRP_OK;
+    if (!idx_dev || !vals_dev) { set_error("idx/vals is NULL"); return MTTKRP_EINVAL; }
+    return launch_export(h, idx_dev, vals_dev, static_cast<cudaStream_t>(cuda_stream));
+}
+
+}  // extern "C"

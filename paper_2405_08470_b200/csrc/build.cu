@@ -1,0 +1,478 @@
+// On-device format builder (mttkrp_create): hand-written stable LSD radix sort of the nonzeros by
+// each mode's key tuple, position maps between consecutive layouts (the paper's remap ids,
+// PAPER.md:185; unique per element, Observation 1 PAPER.md:297-299), the mode-0 tensor copy
+// (PAPER.md:145), and per-mode tables (empty output rows; rows that span shards).
+// The paper builds its format on the CPU (Sec. 5.7); here it is done on the GPU.
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <algorithm>
+#include "common.cuh"
+
+namespace mk {
+
+// ----------------------------------------------------------------------------------------------
+// workspace plan
+// ----------------------------------------------------------------------------------------------
+static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+constexpr int kSortThreads = 256;
+constexpr int kSortItems = 16;
+constexpr int kSortTile = kSortThreads * kSortItems;   // keys per block per radix pass
+constexpr int kScanThreads = 256;
+constexpr int kScanItems = 8;
+constexpr int kScanTile = kScanThreads * kScanItems;
+
+static int choose_shard_nnz(int64_t nnz) {
+    // Aim for >= 8 shards per SM on 148 SMs; power of two in [kMinShardNnz, kMaxShardNnz].
+    int s = kMaxShardNnz;
+    while (s > kMinShardNnz && nnz / s < 148 * 8) s >>= 1;
+    return s;
+}
+
+mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_rank, WorkspacePlan* p) {
+    memset(p, 0, sizeof(*p));
+    const size_t n = (size_t)nnz;
+    const size_t rec_bytes = (size_t)(N + 1) * 4 * n;
+    p->shard_nnz = choose_shard_nnz(nnz);
+    p->num_shards = (nnz + p->shard_nnz - 1) / p->shard_nnz;
+    size_t off = 0;
+    p->rec_a = off; off = align_up(off + rec_bytes);
+    for (int d = 0; d < N; ++d) { p->next[d] = off; off = align_up(off + 4 * n); }
+    p->perm0 = off; off = align_up(off + 4 * n);
+    for (int d = 0; d < N; ++d) { p->empty[d] = off; off = align_up(off + 4 * (size_t)dims[d]); }
+    for (int d = 0; d < N; ++d) { p->chains[d] = off; off = align_up(off + 12 * (size_t)p->num_shards); }
+    p->carry = off; off = align_up(off + (size_t)2 * p->num_shards * kMaxRank * 4);
+    if (max_rank > 0) {
+        for (int d = 0; d < N; ++d) { p->stage_fac[d] = off; off = align_up(off + (size_t)dims[d] * max_rank * 4); }
+        for (int d = 0; d < N; ++d) { p->stage_out[d] = off; off = align_up(off + (size_t)dims[d] * max_rank * 4); }
+    }
+    p->persistent_end = off;
+    p->rec_b = off;
+    p->scratch = off;
+    int64_t maxdim = 1;
+    for (int d = 0; d < N; ++d) maxdim = std::max<int64_t>(maxdim, dims[d]);
+    const size_t nblocks = (n + kSortTile - 1) / kSortTile;
+    size_t scratch = 0;
+    scratch += 4 * align_up(4 * n);                                   // key/perm ping-pong
+    scratch += align_up(4 * (256 * nblocks + 1));                     // digit histogram table
+    scratch += 2 * align_up(4 * ((size_t)std::max<int64_t>(maxdim, p->num_shards) + 1));   // flags + positions
+    scratch += align_up(4 * (std::max<size_t>(256 * nblocks + 1, (size_t)maxdim + 1) / kScanTile + 2));  // scan block sums
+    scratch += 4096;                                                  // counters, error flag
+    p->total = off + std::max(align_up(rec_bytes), scratch);
+    return MTTKRP_OK;
+}
+
+// ----------------------------------------------------------------------------------------------
+// small kernels
+// ----------------------------------------------------------------------------------------------
+__global__ void k_validate(const int32_t* __restrict__ idx, int64_t nnz, int N, const int64_t* __restrict__ dims_dev,
+                           uint32_t* __restrict__ bad) {
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int m = blockIdx.y;
+    if (k < nnz) {
+        int32_t v = idx[(size_t)m * nnz + k];
+        if (v < 0 || (int64_t)v >= dims_dev[m]) atomicOr(bad, 1u << m);
+    }
+}
+
+__global__ void k_iota(uint32_t* __restrict__ p, int64_t n) {
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) p[k] = (uint32_t)k;
+}
+
+// key[k] = col[perm[k]]
+__global__ void k_gather_u32(const uint32_t* __restrict__ col, const uint32_t* __restrict__ perm,
+                             uint32_t* __restrict__ key, int64_t n) {
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) key[k] = col[perm[k]];
+}
+
+// p[k] = table[p[k]] (in place)
+__global__ void k_apply_table(const uint32_t* __restrict__ table, uint32_t* p, int64_t n) {
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) p[k] = table[p[k]];
+}
+
+// inv[perm[j]] = j
+__global__ void k_invert(const uint32_t* __restrict__ perm, uint32_t* __restrict__ inv, int64_t n) {
+    int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j < n) inv[perm[j]] = (uint32_t)j;
+}
+
+// ----------------------------------------------------------------------------------------------
+// exclusive scan (uint32), three phases; in and out may alias
+// ----------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* total, uint32_t* smem /*>=33*/) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) smem[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        uint32_t w = (lane < (int)(blockDim.x >> 5)) ? smem[lane] : 0;
+        uint32_t winc = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t t = __shfl_up_sync(0xffffffffu, winc, o);
+            if (lane >= o) winc += t;
+        }
+        smem[lane] = winc - w;
+        if (lane == 31) smem[32] = winc;
+    }
+    __syncthreads();
+    uint32_t res = smem[warp] + inc - v;
+    *total = smem[32];
+    __syncthreads();
+    return res;
+}
+
+__global__ void __launch_bounds__(kScanThreads) k_scan_reduce(const uint32_t* __restrict__ in, int64_t n,
+                                                              uint32_t* __restrict__ sums) {
+    __shared__ uint32_t sm[33];
+    int64_t base = (int64_t)blockIdx.x * kScanTile + (int64_t)threadIdx.x * kScanItems;
+    uint32_t s = 0;
+#pragma unroll
+    for (int i = 0; i < kScanItems; ++i)
+        if (base + i < n) s += in[base + i];
+    uint32_t tot;
+    block_exclusive_scan(s, &tot, sm);
+    if (threadIdx.x == 0) sums[blockIdx.x] = tot;
+}
+
+__global__ void __launch_bounds__(1024) k_scan_sums(uint32_t* __restrict__ sums, int64_t nb) {
+    __shared__ uint32_t sm[33];
+    uint32_t carry = 0;
+    for (int64_t base = 0; base < nb; base += 1024) {
+        int64_t i = base + threadIdx.x;
+        uint32_t v = (i < nb) ? sums[i] : 0;
+        uint32_t tot;
+        uint32_t ex = block_exclusive_scan(v, &tot, sm);
+        if (i < nb) sums[i] = carry + ex;
+        carry += tot;
+    }
+}
+
+__global__ void __launch_bounds__(kScanThreads) k_scan_apply(const uint32_t* in, uint32_t* out, int64_t n,
+                                                             const uint32_t* __restrict__ sums) {
+    __shared__ uint32_t sm[33];
+    int64_t base = (int64_t)blockIdx.x * kScanTile + (int64_t)threadIdx.x * kScanItems;
+    uint32_t v[kScanItems];
+    uint32_t s = 0;
+#pragma unroll
+    for (int i = 0; i < kScanItems; ++i) {
+        v[i] = (base + i < n) ? in[base + i] : 0;
+        s += v[i];
+    }
+    uint32_t tot;
+    uint32_t ex = block_exclusive_scan(s, &tot, sm) + sums[blockIdx.x];
+#pragma unroll
+    for (int i = 0; i < kScanItems; ++i) {
+        if (base + i < n) out[base + i] = ex;
+        ex += v[i];
+    }
+}
+
+static mttkrp_status_t exclusive_scan(uint32_t* data, int64_t n, uint32_t* sums, cudaStream_t st) {
+    if (n <= 0) return MTTKRP_OK;
+    int64_t nb = (n + kScanTile - 1) / kScanTile;
+    k_scan_reduce<<<(unsigned)nb, kScanThreads, 0, st>>>(data, n, sums);
+    k_scan_sums<<<1, 1024, 0, st>>>(sums, nb);
+    k_scan_apply<<<(unsigned)nb, kScanThreads, 0, st>>>(data, data, n, sums);
+    MK_CUDA(cudaGetLastError());
+    return MTTKRP_OK;
+}
+
+// ----------------------------------------------------------------------------------------------
+// stable LSD radix pass over (key, payload) pairs, 8-bit digits
+// ----------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kSortThreads) k_radix_hist(const uint32_t* __restrict__ keys, int64_t n, int shift,
+                                                             uint32_t* __restrict__ hist, int64_t nblocks) {
+    __shared__ uint32_t cnt[256];
+    cnt[threadIdx.x] = 0;
+    __syncthreads();
+    int64_t base = (int64_t)blockIdx.x * kSortTile;
+#pragma unroll
+    for (int i = 0; i < kSortItems; ++i) {
+        int64_t k = base + (int64_t)i * kSortThreads + threadIdx.x;
+        if (k < n) atomicAdd(&cnt[(keys[k] >> shift) & 255u], 1u);
+    }
+    __syncthreads();
+    hist[(size_t)threadIdx.x * nblocks + blockIdx.x] = cnt[threadIdx.x];
+}
+
+// Block b owns keys [b*tile, (b+1)*tile); warp w owns a contiguous 32*items slice of it, item i of
+// lane l being element slice + i*32 + l.  Ranks are assigned in exactly that memory order, so equal
+// digits keep their input order (stability).
+__global__ void __launch_bounds__(kSortThreads) k_radix_scatter(const uint32_t* __restrict__ keys_in,
+                                                                const uint32_t* __restrict__ vals_in,
+                                                                uint32_t* __restrict__ keys_out,
+                                                                uint32_t* __restrict__ vals_out, int64_t n, int shift,
+                                                                const uint32_t* __restrict__ offs, int64_t nblocks) {
+    constexpr int kWarps = kSortThreads / 32;
+    __shared__ uint32_t cnt[kWarps][256];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int i = threadIdx.x; i < kWarps * 256; i += kSortThreads) (&cnt[0][0])[i] = 0;
+    __syncthreads();
+    const int64_t base = (int64_t)blockIdx.x * kSortTile + (int64_t)warp * (32 * kSortItems);
+    uint32_t key[kSortItems], val[kSortItems], rnk[kSortItems];
+    const unsigned lt = (1u << lane) - 1u;
+#pragma unroll
+    for (int i = 0; i < kSortItems; ++i) {
+        int64_t k = base + i * 32 + lane;
+        bool valid = k < n;
+        key[i] = valid ? keys_in[k] : 0u;
+        val[i] = valid ? vals_in[k] : 0u;
+        unsigned dig = valid ? ((key[i] >> shift) & 255u) : 256u;
+        unsigned peers = __match_any_sync(0xffffffffu, dig);
+        unsigned before = __popc(peers & lt);
+        uint32_t old = 0;
+        if (valid) old = cnt[warp][dig];
+        __syncwarp();
+        if (valid && before == 0) cnt[warp][dig] = old + __popc(peers);
+        __syncwarp();
+        rnk[i] = old + before;
+    }
+    __syncthreads();
+    {
+        const int dig = threadIdx.x;   // kSortThreads == 256 digits
+        uint32_t run = offs[(size_t)dig * nblocks + blockIdx.x];
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) {
+            uint32_t c = cnt[w][dig];
+            cnt[w][dig] = run;
+            run += c;
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < kSortItems; ++i) {
+        int64_t k = base + i * 32 + lane;
+        if (k < n) {
+            unsigned dig = (key[i] >> shift) & 255u;
+            uint32_t pos = cnt[warp][dig] + rnk[i];
+            keys_out[pos] = key[i];
+            vals_out[pos] = val[i];
+        }
+    }
+}
+
+// ----------------------------------------------------------------------------------------------
+// records, maps, tables
+// ----------------------------------------------------------------------------------------------
+// rec[k] = { idx[order[0]][perm[k]], ..., idx[order[N-1]][perm[k]], val[perm[k]] }
+struct OrderArg { int v[kMaxModes]; };
+
+__global__ void k_build_records(const int32_t* __restrict__ idx, const float* __restrict__ vals,
+                                const uint32_t* __restrict__ perm, int64_t nnz, int N, OrderArg order,
+                                uint32_t* __restrict__ rec) {
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nnz) return;
+    uint32_t src = perm[k];
+    uint32_t* r = rec + (size_t)k * (N + 1);
+    for (int l = 0; l < N; ++l) r[l] = (uint32_t)idx[(size_t)order.v[l] * nnz + src];
+    r[N] = __float_as_uint(vals[src]);
+}
+
+__global__ void k_mark_rows(const uint32_t* __restrict__ kd, int64_t nnz, uint32_t* __restrict__ present) {
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < nnz) present[kd[k]] = 1u;
+}
+
+// flags[i] = 1 - present[i] for i < rows, flags[rows] = 0
+__global__ void k_invert_flags(uint32_t* __restrict__ flags, int64_t rows) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < rows) flags[i] = 1u - flags[i];
+    else if (i == rows) flags[i] = 0u;
+}
+
+// After the exclusive scan pos[] of the flags: compact the flagged ids.  A flagged id i has
+// pos[i+1] == pos[i] + 1.
+__global__ void k_compact_ids(const uint32_t* __restrict__ pos, int64_t n, uint32_t* __restrict__ list) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n && pos[i + 1] != pos[i]) list[pos[i]] = (uint32_t)i;
+}
+
+// Shard s covers positions [s*S, min((s+1)*S, nnz)).  A chain starts at s when the last row of s
+// continues into s+1 and that row begins inside s.
+__global__ void k_chain_flags(const uint32_t* __restrict__ kd, int64_t nnz, int S, int64_t nshards,
+                              uint32_t* __restrict__ flags) {
+    int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s > nshards) return;
+    if (s == nshards) { flags[s] = 0; return; }
+    int64_t end = min((s + 1) * (int64_t)S, nnz);
+    uint32_t f = 0;
+    if (end < nnz) {
+        uint32_t r = kd[end - 1];
+        if (kd[end] == r) f = (s == 0 || kd[s * (int64_t)S - 1] != r) ? 1u : 0u;
+    }
+    flags[s] = f;
+}
+
+__global__ void k_chain_fill(const uint32_t* __restrict__ kd, int64_t nnz, int S, int64_t nshards,
+                             const uint32_t* __restrict__ pos, uint32_t* __restrict__ chains) {
+    int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= nshards || pos[s + 1] == pos[s]) return;
+    int64_t end = min((s + 1) * (int64_t)S, nnz);
+    uint32_t r = kd[end - 1];
+    // upper bound of r in kd[end, nnz)
+    int64_t lo = end, hi = nnz;
+    while (lo < hi) {
+        int64_t mid = (lo + hi) >> 1;
+        if (kd[mid] <= r) lo = mid + 1; else hi = mid;
+    }
+    uint32_t* c = chains + (size_t)pos[s] * 3;
+    c[0] = (uint32_t)s;
+    c[1] = (uint32_t)((lo - 1) / S);
+    c[2] = r;
+}
+
+static inline unsigned grid_for(int64_t n, int threads) { return (unsigned)std::max<int64_t>(1, (n + threads - 1) / threads); }
+
+static int ceil_log2_i64(int64_t x) {
+    int b = 0;
+    while (((int64_t)1 << b) < x) ++b;
+    return b;
+}
+
+void choose_key_order(int N, const int64_t* dims, int d, int* order) {
+    // order[0] = d; the other modes by descending size (ties: lower mode first), so the largest
+    // input factor is the one reused along a fiber and the smallest, most cacheable one is the
+    // per-nonzero gather (reading 4).  MTTKRP_KEY_ORDER=asc|cyclic overrides (tuning).
+    const char* env = getenv("MTTKRP_KEY_ORDER");
+    int rest[kMaxModes], n = 0;
+    for (int j = 1; j < N; ++j) rest[n++] = (d + j) % N;     // cyclic
+    if (!env || strcmp(env, "cyclic") != 0) {
+        bool asc = env && strcmp(env, "asc") == 0;
+        std::sort(rest, rest + n, [&](int a, int b) {
+            if (dims[a] != dims[b]) return asc ? dims[a] < dims[b] : dims[a] > dims[b];
+            return a < b;
+        });
+    }
+    order[0] = d;
+    for (int j = 0; j < n; ++j) order[j + 1] = rest[j];
+}
+
+mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char* ws, const int32_t* idx,
+                             const float* vals, cudaStream_t st) {
+    const int N = h->N;
+    const int64_t nnz = h->nnz;
+    const size_t n = (size_t)nnz;
+    const int S = h->shard_nnz;
+    const int64_t nshards = h->num_shards;
+    int64_t maxdim = 1;
+    for (int d = 0; d < N; ++d) maxdim = std::max<int64_t>(maxdim, h->dims[d]);
+    const int64_t nblocks = (nnz + kSortTile - 1) / kSortTile;
+
+    // scratch carve-up (mirrors plan_workspace)
+    char* sp = ws + plan.scratch;
+    auto take = [&](size_t bytes) { char* p = sp; sp += align_up(bytes); return p; };
+    uint32_t* keyA = (uint32_t*)take(4 * n);
+    uint32_t* keyB = (uint32_t*)take(4 * n);
+    uint32_t* permA = (uint32_t*)take(4 * n);
+    uint32_t* permB = (uint32_t*)take(4 * n);
+    uint32_t* hist = (uint32_t*)take(4 * (256 * (size_t)nblocks + 1));
+    const size_t flag_n = (size_t)std::max<int64_t>(maxdim, nshards) + 1;
+    uint32_t* flags = (uint32_t*)take(4 * flag_n);
+    uint32_t* flags2 = (uint32_t*)take(4 * flag_n);
+    (void)flags2;
+    uint32_t* sums = (uint32_t*)take(4 * (std::max<size_t>(256 * (size_t)nblocks + 1, (size_t)maxdim + 1) / kScanTile + 2));
+    uint32_t* small = (uint32_t*)take(4096);          // [0]=bad flag, [8..8+2N) counts, then dims
+    int64_t* dims_dev = (int64_t*)(small + 64);
+
+    MK_CUDA(cudaMemsetAsync(small, 0, 4096, st));
+    MK_CUDA(cudaMemcpyAsync(dims_dev, h->dims, sizeof(int64_t) * N, cudaMemcpyHostToDevice, st));
+
+    if (nnz > 0) {
+        dim3 g(grid_for(nnz, 256), N);
+        k_validate<<<g, 256, 0, st>>>(idx, nnz, N, dims_dev, small);
+        MK_CUDA(cudaGetLastError());
+        uint32_t bad = 0;
+        MK_CUDA(cudaMemcpyAsync(&bad, small, 4, cudaMemcpyDeviceToHost, st));
+        MK_CUDA(cudaStreamSynchronize(st));
+        if (bad) {
+            set_error("index out of range in mode mask 0x%x", bad);
+            return MTTKRP_EINDEX;
+        }
+    }
+
+    for (int d = 0; d < N; ++d) {
+        ModeMeta& mm = h->mode[d];
+        uint32_t* dst = mm.next;   // holds perm_d until the maps are built
+        if (nnz > 0) {
+            uint32_t *ka = keyA, *kb = keyB, *pa = permA, *pb = permB;
+            k_iota<<<grid_for(nnz, 256), 256, 0, st>>>(pa, nnz);
+            for (int j = N - 1; j >= 0; --j) {
+                const int m = mm.order[j];
+                const uint32_t* col = (const uint32_t*)idx + (size_t)m * n;
+                k_gather_u32<<<grid_for(nnz, 256), 256, 0, st>>>(col, pa, ka, nnz);
+                const int bits = ceil_log2_i64(h->dims[m]);
+                for (int shift = 0; shift < bits; shift += 8) {
+                    k_radix_hist<<<(unsigned)nblocks, kSortThreads, 0, st>>>(ka, nnz, shift, hist, nblocks);
+                    MK_TRY(exclusive_scan(hist, 256 * nblocks, sums, st));
+                    k_radix_scatter<<<(unsigned)nblocks, kSortThreads, 0, st>>>(ka, pa, kb, pb, nnz, shift, hist, nblocks);
+                    std::swap(ka, kb);
+                    std::swap(pa, pb);
+                }
+                MK_CUDA(cudaGetLastError());
+            }
+            // pa = perm_d, ka = idx[d] in mode-d order
+            MK_CUDA(cudaMemcpyAsync(dst, pa, 4 * n, cudaMemcpyDeviceToDevice, st));
+            if (d == 0) MK_CUDA(cudaMemcpyAsync(h->perm0, pa, 4 * n, cudaMemcpyDeviceToDevice, st));
+
+            // split rows (chains)
+            if (nshards > 0) {
+                k_chain_flags<<<grid_for(nshards + 1, 256), 256, 0, st>>>(ka, nnz, S, nshards, flags);
+                MK_TRY(exclusive_scan(flags, nshards + 1, sums, st));
+                k_chain_fill<<<grid_for(nshards, 256), 256, 0, st>>>(ka, nnz, S, nshards, flags, mm.chains);
+                MK_CUDA(cudaMemcpyAsync(small + 8 + 2 * d, flags + nshards, 4, cudaMemcpyDeviceToDevice, st));
+            }
+            // empty rows
+            const int64_t rows = h->dims[d];
+            MK_CUDA(cudaMemsetAsync(flags, 0, 4 * (size_t)(rows + 1), st));
+            k_mark_rows<<<grid_for(nnz, 256), 256, 0, st>>>(ka, nnz, flags);
+            k_invert_flags<<<grid_for(rows + 1, 256), 256, 0, st>>>(flags, rows);
+            MK_TRY(exclusive_scan(flags, rows + 1, sums, st));
+            k_compact_ids<<<grid_for(rows, 256), 256, 0, st>>>(flags, rows, mm.empty_rows);
+            MK_CUDA(cudaMemcpyAsync(small + 8 + 2 * d + 1, flags + rows, 4, cudaMemcpyDeviceToDevice, st));
+            MK_CUDA(cudaGetLastError());
+        } else {
+            // no nonzeros: every row is empty
+            const int64_t rows = h->dims[d];
+            k_iota<<<grid_for(rows, 256), 256, 0, st>>>(mm.empty_rows, rows);
+            MK_CUDA(cudaGetLastError());
+        }
+    }
+
+    if (nnz > 0) {
+        // tensor copy in mode-0 order
+        OrderArg oa;
+        for (int l = 0; l < kMaxModes; ++l) oa.v[l] = h->mode[0].order[l];
+        k_build_records<<<grid_for(nnz, 256), 256, 0, st>>>(idx, vals, h->perm0, nnz, N, oa, h->rec_cur);
+        // next_d[k] = inv_{d+1}[perm_d[k]]; slot d still holds perm_d; go d = 0..N-1, the last one
+        // needs perm_0 which slot 0 no longer holds -> use the perm0 copy.
+        uint32_t* inv = keyA;
+        for (int d = 0; d < N; ++d) {
+            const int e = (d + 1) % N;
+            const uint32_t* perm_e = (e == 0) ? h->perm0 : h->mode[e].next;
+            k_invert<<<grid_for(nnz, 256), 256, 0, st>>>(perm_e, inv, nnz);
+            k_apply_table<<<grid_for(nnz, 256), 256, 0, st>>>(inv, h->mode[d].next, nnz);
+        }
+        MK_CUDA(cudaGetLastError());
+    }
+
+    uint32_t counts[2 * kMaxModes] = {0};
+    MK_CUDA(cudaMemcpyAsync(counts, small + 8, sizeof(uint32_t) * 2 * N, cudaMemcpyDeviceToHost, st));
+    MK_CUDA(cudaStreamSynchronize(st));
+    for (int d = 0; d < N; ++d) {
+        h->mode[d].n_chains = nnz > 0 ? counts[2 * d] : 0;
+        h->mode[d].n_empty = nnz > 0 ? counts[2 * d + 1] : h->dims[d];
+    }
+    return MTTKRP_OK;
+}
+
+}  // namespace mk

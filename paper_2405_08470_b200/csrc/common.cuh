@@ -1,0 +1,93 @@
+// Internal declarations shared by the translation units of libmttkrp_b200 (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/mttkrp.h"
+
+namespace mk {
+
+constexpr int kMaxModes = MTTKRP_MAX_MODES;
+constexpr int kMaxShardNnz = 8192;   // nonzeros per thread-block shard (upper bound)
+constexpr int kMinShardNnz = 1024;
+constexpr int kMaxRank = 64;
+constexpr int kBlockThreads = 256;   // MTTKRP kernel: 8 warps
+
+void set_error(const char* fmt, ...);
+
+#define MK_CUDA(call)                                                                        \
+    do {                                                                                     \
+        cudaError_t e__ = (call);                                                            \
+        if (e__ != cudaSuccess) {                                                            \
+            mk::set_error("%s:%d %s -> %s", __FILE__, __LINE__, #call, cudaGetErrorString(e__)); \
+            return MTTKRP_ECUDA;                                                             \
+        }                                                                                    \
+    } while (0)
+
+#define MK_TRY(expr)                              \
+    do {                                          \
+        mttkrp_status_t s__ = (expr);             \
+        if (s__ != MTTKRP_OK) return s__;         \
+    } while (0)
+
+// Per-mode tables built by mttkrp_create.
+struct ModeMeta {
+    int order[kMaxModes];     // sort-key order of this layout, order[0] == mode
+    int pos[kMaxModes];       // pos[m] = level of mode m in `order`
+    uint32_t* next;           // [nnz] position in layout (d+1)%N of the element at position k here
+    uint32_t* empty_rows;     // [n_empty] output rows without a nonzero
+    int64_t n_empty;
+    uint32_t* chains;         // [n_chains][3] = {first shard, last shard, row} for rows spanning shards
+    int64_t n_chains;
+};
+
+}  // namespace mk
+
+struct mttkrp_handle_s {
+    int N;
+    int64_t dims[mk::kMaxModes];
+    int64_t nnz;
+    int rec_words;            // N + 1 (N role-ordered int32 indices, then the fp32 value)
+    int shard_nnz;
+    int64_t num_shards;
+    uint32_t* rec_cur;        // resident tensor copy T_in, layout `cur`
+    uint32_t* rec_alt;        // T_out
+    uint32_t* perm0;          // [nnz] original COO position of element k of layout 0
+    mk::ModeMeta mode[mk::kMaxModes];
+    float* carry;             // [2*num_shards][kMaxRank] partial rows of split rows
+    int cur;
+    int max_rank;
+    float* stage_fac[mk::kMaxModes];
+    float* stage_out[mk::kMaxModes];
+    int64_t bytes_held;
+    int64_t remaps_done;
+    int device;
+};
+
+namespace mk {
+
+// ---- build.cu -------------------------------------------------------------------------------
+struct WorkspacePlan {
+    size_t rec_a, rec_b, perm0, carry;
+    size_t next[kMaxModes], empty[kMaxModes], chains[kMaxModes];
+    size_t stage_fac[kMaxModes], stage_out[kMaxModes];
+    size_t persistent_end;
+    size_t scratch;          // start of the create-time scratch (may overlap rec_b)
+    size_t total;
+    int shard_nnz;
+    int64_t num_shards;
+};
+mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_rank, WorkspacePlan* p);
+mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char* ws,
+                             const int32_t* idx, const float* vals, cudaStream_t st);
+
+// ---- remap.cu -------------------------------------------------------------------------------
+mttkrp_status_t launch_remap(mttkrp_handle_s* h, int from, cudaStream_t st);   // from -> (from+1)%N, swaps copies
+mttkrp_status_t launch_export(const mttkrp_handle_s* h, int32_t* idx, float* vals, cudaStream_t st);
+mttkrp_status_t launch_perm_step(const uint32_t* next, const uint32_t* in, uint32_t* out, int64_t nnz, cudaStream_t st);
+
+// ---- mttkrp_kernel.cu -----------------------------------------------------------------------
+mttkrp_status_t launch_mttkrp(const mttkrp_handle_s* h, int d, const float* const* factors, int R,
+                              float* out, cudaStream_t st);
+
+}  // namespace mk

@@ -1,0 +1,190 @@
+"""GPU parity: the CUDA path (through the C-ABI, via the ctypes binding) against the fp64 oracle,
+element by element, on the same seeded inputs.
+
+Bars (BASELINE.json north_star):
+  * remap permutation and remapped tensor copy: bit-exact against the oracle's stable sort;
+  * Y_d: max |Y_gpu - Y_oracle| / S_d <= 1e-5 with S_d = sum |val| prod |A_m| per entry, and entries
+    with S_d == 0 exactly 0.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-5
+
+
+@pytest.fixture(scope="module")
+def P():
+    import paper_2405_08470_b200 as pkg
+    pkg.load_library()          # fails loudly if the CUDA library is missing
+    assert torch.cuda.is_available()
+    return pkg
+
+
+def _run_case(P, dims, idx_cpu, vals_cpu, R, seed, order_modes=None, check_perm=True, ones=False):
+    N = len(dims)
+    dev = torch.device("cuda:0")
+    rng = np.random.default_rng(seed)
+    if ones:
+        fac_np = [np.ones((d, R), dtype=np.float32) for d in dims]
+    else:
+        fac_np = [rng.uniform(-1, 1, size=(d, R)).astype(np.float32) for d in dims]
+    fac = [torch.from_numpy(f).to(dev) for f in fac_np]
+    h = P.Mttkrp(dims, idx_cpu.to(dev), vals_cpu.to(dev))
+    info = h.info()
+    assert info["cur_layout"] == 0 and info["nnz"] == vals_cpu.numel()
+    idx_np, vals_np = idx_cpu.numpy(), vals_cpu.numpy()
+    perms = {}
+    if check_perm and vals_cpu.numel() > 0:
+        for d in range(N):
+            order = info["key_order"][d]
+            assert order[0] == d and sorted(order) == list(range(N))
+            perms[d] = oracle.sort_perm(dims, idx_np, order)
+            got = h.get_perm(d).cpu().numpy().astype(np.int64)
+            np.testing.assert_array_equal(got, perms[d])            # bit-exact (Observation 1: a bijection)
+    modes = list(order_modes) if order_modes is not None else list(range(N))
+    worst = 0.0
+    for d in modes:
+        Y = h.mttkrp_mode(d, fac).cpu().numpy()
+        assert h.info()["cur_layout"] == d
+        if d in perms:                                                # remapped copy is the sorted COO
+            gi, gv = h.export_coo()
+            np.testing.assert_array_equal(gi.cpu().numpy(), idx_np[:, perms[d]])
+            np.testing.assert_array_equal(gv.cpu().numpy(), vals_np[perms[d]])
+        Yo, So = oracle.mttkrp_mode(dims, idx_np, vals_np, fac_np, d, perm=perms.get(d))
+        err, zeros_ok = oracle.normalised_error(Y, Yo, So)
+        assert zeros_ok, f"mode {d}: entries without contributions must be exactly 0"
+        assert err <= TOL, f"mode {d}: normalised error {err:.3e} > {TOL}"
+        worst = max(worst, err)
+    h.destroy()
+    return worst, info
+
+
+@pytest.mark.parametrize("dims,nnz,dup", [((4, 3, 5), 30, False), ((3, 4, 2, 3), 40, True), ((2, 3, 2, 2, 3), 50, False),
+                                          ((5, 4), 12, True), ((7, 1, 3), 15, False), ((2, 2, 2, 2, 2, 2), 40, True),
+                                          ((3, 2, 2, 2, 2, 2, 2), 60, True), ((2, 2, 2, 3, 2, 2, 2, 2), 80, True)])
+@pytest.mark.parametrize("R", [8, 32])
+def test_tiny_tensors(P, dims, nnz, dup, R):
+    t = W.tiny_tensor(dims, nnz, seed=len(dims) * 100 + nnz, duplicates=dup)
+    _run_case(P, list(dims), t.idx, t.vals, R, seed=1)
+
+
+@pytest.mark.parametrize("R", [8, 16, 32, 64])
+def test_config1_full(P, R):
+    # BASELINE.json configs[0] at full size (R=16 is the config's rank; the others widen it).
+    spec = W.CONFIGS[0]
+    t = W.generate_tensor(spec)
+    worst, info = _run_case(P, spec.dims, t.idx, t.vals, R, seed=2)
+    assert info["num_shards"] > 1
+
+
+@pytest.mark.parametrize("cfg,nnz,R", [(1, 300_000, 32), (2, 300_000, 32), (3, 250_000, 32), (4, 200_000, 8),
+                                       (4, 200_000, 16), (4, 200_000, 32), (4, 200_000, 64)])
+def test_scaled_configs(P, cfg, nnz, R):
+    # Shape classes of configs 2-5 (Zipf skew, tiny and huge modes) at sizes the oracle does in
+    # seconds; nnz is not a multiple of the shard size (ragged tail) and spans many shards.
+    spec = W.CONFIGS[cfg].scaled(nnz + 137)
+    t = W.generate_tensor(spec)
+    worst, info = _run_case(P, spec.dims, t.idx, t.vals, R, seed=3)
+    assert info["num_shards"] >= 30
+    assert max(info["num_split_rows"]) > 0          # skewed modes do have rows spanning shards
+
+
+def test_heavy_rows_span_many_shards(P):
+    # Degenerate: a mode with 2 rows (the paper's Vast tensor has one) and a mode of size 1.
+    dims = [2, 50, 1, 400]
+    spec = W.TensorSpec("heavy", dims, 30_000, [0.0, 0.0, 0.0, 0.0], "uniform", (32,), 77)
+    t = W.generate_tensor(spec)
+    worst, info = _run_case(P, dims, t.idx, t.vals, 32, seed=4)
+    assert info["num_split_rows"][0] >= 1 and info["num_split_rows"][2] == 1
+
+
+def test_all_ones_closed_form(P):
+    # All-ones dense tensor and factors: Y_d[i, r] = prod_{m != d} I_m exactly (fp32 below 2^24).
+    dims = [12, 9, 11]
+    grid = np.stack(np.meshgrid(*[np.arange(d) for d in dims], indexing="ij")).reshape(3, -1).astype(np.int32)
+    rng = np.random.default_rng(0)
+    grid = grid[:, rng.permutation(grid.shape[1])]
+    idx = torch.from_numpy(np.ascontiguousarray(grid))
+    vals = torch.ones(idx.shape[1], dtype=torch.float32)
+    dev = torch.device("cuda:0")
+    h = P.Mttkrp(dims, idx.to(dev), vals.to(dev))
+    fac = [torch.ones((d, 16), dtype=torch.float32, device=dev) for d in dims]
+    for d in range(3):
+        Y = h.mttkrp_mode(d, fac).cpu().numpy()
+        want = np.prod([dims[m] for m in range(3) if m != d])
+        assert np.all(Y == float(want))
+    h.destroy()
+
+
+def test_any_order_and_repeat(P):
+    # Layouts are history-free (reading 5): any call order gives the same result.
+    spec = W.CONFIGS[0].scaled(20_011)
+    t = W.generate_tensor(spec)
+    _run_case(P, spec.dims, t.idx, t.vals, 16, seed=5, order_modes=[2, 2, 0, 1, 0, 2, 1, 1], check_perm=True)
+
+
+def test_empty_tensor_and_empty_rows(P):
+    dev = torch.device("cuda:0")
+    dims = [5, 4, 3]
+    h = P.Mttkrp(dims, torch.empty((3, 0), dtype=torch.int32, device=dev), torch.empty(0, dtype=torch.float32, device=dev))
+    fac = [torch.rand((d, 8), device=dev) for d in dims]
+    for d in range(3):
+        out = torch.full((dims[d], 8), float("nan"), device=dev)
+        h.mttkrp_mode(d, fac, out=out)
+        assert torch.all(out == 0)
+    assert h.info()["num_empty_rows"] == dims
+    h.destroy()
+    # one nonzero in a large mode: every other row must be overwritten with zeros (NaN-poisoned out)
+    dims = [1000, 3, 2]
+    idx = torch.tensor([[777], [1], [0]], dtype=torch.int32, device=dev)
+    vals = torch.tensor([2.0], device=dev)
+    h = P.Mttkrp(dims, idx, vals)
+    fac = [torch.full((d, 32), 0.5, device=dev) for d in dims]
+    out = torch.full((1000, 32), float("nan"), device=dev)
+    h.mttkrp_mode(0, fac, out=out)
+    assert torch.all(out[777] == 0.5) and torch.all(out[:777] == 0) and torch.all(out[778:] == 0)
+    h.destroy()
+
+
+def test_sweep_and_host_entry_points(P):
+    spec = W.CONFIGS[0].scaled(50_021)
+    t = W.generate_tensor(spec)
+    dev = torch.device("cuda:0")
+    R = 16
+    fac_cpu = W.generate_factors(spec, R)
+    fac = [f.to(dev) for f in fac_cpu]
+    h = P.Mttkrp(spec.dims, t.idx.to(dev), t.vals.to(dev), max_rank=R)
+    outs = h.mttkrp_sweep(fac)
+    fac_pin = [f.pin_memory() for f in fac_cpu]
+    outs_host = [torch.empty((d, R), dtype=torch.float32).pin_memory() for d in spec.dims]
+    h.mttkrp_sweep_host(fac_pin, outs_host)
+    for d in range(3):
+        assert torch.equal(outs[d].cpu(), outs_host[d])            # same kernels, same order: bit-identical
+        Yo, So = oracle.mttkrp_mode(spec.dims, t.idx.numpy(), t.vals.numpy(), [f.numpy() for f in fac_cpu], d)
+        err, zeros_ok = oracle.normalised_error(outs[d].cpu().numpy(), Yo, So)
+        assert zeros_ok and err <= TOL
+    assert h.info()["remaps_done"] == 5          # 0->1->2 (sweep), 2->0->1->2 (host sweep): 2 + 3
+    h.destroy()
+
+
+def test_errors_are_reported(P):
+    dev = torch.device("cuda:0")
+    dims = [5, 4, 3]
+    idx = torch.tensor([[0, 5], [1, 1], [2, 2]], dtype=torch.int32, device=dev)      # 5 is out of range in mode 0
+    vals = torch.ones(2, device=dev)
+    with pytest.raises(P.MttkrpError) as e:
+        P.Mttkrp(dims, idx, vals)
+    assert e.value.status == 2          # MTTKRP_EINDEX
+    idx[0, 1] = 4
+    h = P.Mttkrp(dims, idx, vals)
+    fac = [torch.rand((d, 12), device=dev) for d in dims]
+    with pytest.raises(P.MttkrpError) as e:
+        h.mttkrp_mode(0, fac)
+    assert e.value.status == 3          # rank 12 unsupported
+    h.destroy()
