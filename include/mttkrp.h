@@ -143,6 +143,19 @@ mttkrp_status_t mttkrp_get_perm(mttkrp_handle_t h, int d, uint32_t* perm_dev, ui
  * [nmodes][nnz] in ORIGINAL mode numbering, device fp32 [nnz]).  Test hook for the remap. */
 mttkrp_status_t mttkrp_export_coo(mttkrp_handle_t h, int32_t* idx_dev, float* vals_dev, void* cuda_stream);
 
+/*
+ * Optional per-kernel-class timing for reports (bench.py's roofline figure).  Between begin and end
+ * the library records a CUDA event pair around every kernel it launches for this handle, on the
+ * stream the kernel is launched on.  end synchronises cuda_stream, sums the elapsed times per class
+ * and stops recording.  Off by default; adds two event records per launch while on.
+ */
+typedef struct {
+    double remap_ms, zero_ms, mttkrp_ms, fixup_ms;                 /* summed device time per kernel class */
+    int64_t remap_launches, zero_launches, mttkrp_launches, fixup_launches;
+} mttkrp_timing_t;
+mttkrp_status_t mttkrp_timing_begin(mttkrp_handle_t h);
+mttkrp_status_t mttkrp_timing_end(mttkrp_handle_t h, mttkrp_timing_t* out /*host*/, void* cuda_stream);
+
 /* Library / build identification, e.g. "mttkrp_b200 0.1 sm_100a". */
 const char* mttkrp_version(void);
 

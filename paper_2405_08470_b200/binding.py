@@ -22,7 +22,7 @@ _STATUS_NAMES = {0: "MTTKRP_OK", 1: "MTTKRP_EINVAL", 2: "MTTKRP_EINDEX", 3: "MTT
 
 EXPORTS = ["mttkrp_workspace_bytes", "mttkrp_create", "mttkrp_mode", "mttkrp_sweep", "mttkrp_remap_to",
            "mttkrp_sweep_host", "mttkrp_destroy", "mttkrp_last_error", "mttkrp_get_info", "mttkrp_get_perm",
-           "mttkrp_export_coo", "mttkrp_version"]
+           "mttkrp_export_coo", "mttkrp_timing_begin", "mttkrp_timing_end", "mttkrp_version"]
 
 
 class MttkrpError(RuntimeError):
@@ -38,6 +38,12 @@ class Info(ctypes.Structure):
                 ("num_split_rows", ctypes.c_int64 * MAX_MODES), ("num_empty_rows", ctypes.c_int64 * MAX_MODES),
                 ("bytes_held", ctypes.c_int64), ("bytes_paper_format", ctypes.c_int64),
                 ("remaps_done", ctypes.c_int64), ("key_order", (ctypes.c_int32 * MAX_MODES) * MAX_MODES)]
+
+
+class Timing(ctypes.Structure):
+    _fields_ = [("remap_ms", ctypes.c_double), ("zero_ms", ctypes.c_double), ("mttkrp_ms", ctypes.c_double),
+                ("fixup_ms", ctypes.c_double), ("remap_launches", ctypes.c_int64), ("zero_launches", ctypes.c_int64),
+                ("mttkrp_launches", ctypes.c_int64), ("fixup_launches", ctypes.c_int64)]
 
 
 _lib = None
@@ -65,6 +71,8 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.mttkrp_get_info.argtypes = [vp, ctypes.POINTER(Info)]
     lib.mttkrp_get_perm.argtypes = [vp, ctypes.c_int, vp, vp, vp]
     lib.mttkrp_export_coo.argtypes = [vp, vp, vp, vp]
+    lib.mttkrp_timing_begin.argtypes = [vp]
+    lib.mttkrp_timing_end.argtypes = [vp, ctypes.POINTER(Timing), vp]
     for name in EXPORTS:
         getattr(lib, name).restype = ctypes.c_int
     lib.mttkrp_last_error.restype = ctypes.c_char_p
@@ -221,6 +229,15 @@ class Mttkrp:
             with torch.cuda.device(self.device):
                 _check(load_library().mttkrp_export_coo(self._h, idx.data_ptr(), vals.data_ptr(), _stream()))
         return idx, vals
+
+    def timing_begin(self) -> None:
+        _check(load_library().mttkrp_timing_begin(self._h))
+
+    def timing_end(self) -> dict:
+        raw = Timing()
+        with torch.cuda.device(self.device):
+            _check(load_library().mttkrp_timing_end(self._h, ctypes.byref(raw), _stream()))
+        return {name: getattr(raw, name) for name, _ in Timing._fields_}
 
     def destroy(self) -> None:
         if getattr(self, "_h", None) is not None and self._h.value:

@@ -101,6 +101,7 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
     h->cur = 0;
     h->max_rank = max_rank;
     h->device = dev;
+    h->timing = new (std::nothrow) Timing();
     for (int d = 0; d < nmodes; ++d) {
         ModeMeta& mm = h->mode[d];
         choose_key_order(nmodes, dims, d, mm.order);
@@ -115,7 +116,7 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
     }
     h->bytes_held = (int64_t)(p.persistent_end + (size_t)(nmodes + 1) * 4 * (size_t)nnz);
     mttkrp_status_t s = build_format(h, p, ws, idx, vals, static_cast<cudaStream_t>(cuda_stream));
-    if (s != MTTKRP_OK) { delete h; return s; }
+    if (s != MTTKRP_OK) { delete h->timing; delete h; return s; }
     *out = h;
     return MTTKRP_OK;
 }
@@ -181,7 +182,41 @@ mttkrp_status_t mttkrp_sweep_host(mttkrp_handle_t h, const float* const* factors
 
 mttkrp_status_t mttkrp_destroy(mttkrp_handle_t h) {
     if (!h) { set_error("handle is NULL"); return MTTKRP_EINVAL; }
+    if (h->timing) {
+        for (auto& e : h->timing->ev) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+        delete h->timing;
+    }
     delete h;
+    return MTTKRP_OK;
+}
+
+mttkrp_status_t mttkrp_timing_begin(mttkrp_handle_t h) {
+    if (!h || !h->timing) { set_error("handle is NULL"); return MTTKRP_EINVAL; }
+    for (auto& e : h->timing->ev) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+    h->timing->ev.clear();
+    h->timing->on = true;
+    return MTTKRP_OK;
+}
+
+mttkrp_status_t mttkrp_timing_end(mttkrp_handle_t h, mttkrp_timing_t* out, void* cuda_stream) {
+    if (!h || !h->timing || !out) { set_error("handle/out is NULL"); return MTTKRP_EINVAL; }
+    h->timing->on = false;
+    memset(out, 0, sizeof(*out));
+    MK_CUDA(cudaStreamSynchronize(static_cast<cudaStream_t>(cuda_stream)));
+    double ms[4] = {0, 0, 0, 0};
+    int64_t cnt[4] = {0, 0, 0, 0};
+    for (auto& e : h->timing->ev) {
+        float t = 0.f;
+        MK_CUDA(cudaEventSynchronize(e.b));
+        MK_CUDA(cudaEventElapsedTime(&t, e.a, e.b));
+        ms[e.cls] += t;
+        cnt[e.cls]++;
+        cudaEventDestroy(e.a);
+        cudaEventDestroy(e.b);
+    }
+    h->timing->ev.clear();
+    out->remap_ms = ms[0]; out->zero_ms = ms[1]; out->mttkrp_ms = ms[2]; out->fixup_ms = ms[3];
+    out->remap_launches = cnt[0]; out->zero_launches = cnt[1]; out->mttkrp_launches = cnt[2]; out->fixup_launches = cnt[3];
     return MTTKRP_OK;
 }
 

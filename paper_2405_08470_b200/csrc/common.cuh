@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stddef.h>
+#include <vector>
 #include "../../include/mttkrp.h"
 
 namespace mk {
@@ -43,6 +44,31 @@ struct ModeMeta {
 
 }  // namespace mk
 
+namespace mk {
+enum KernelClass { kClsRemap = 0, kClsZero = 1, kClsMttkrp = 2, kClsFixup = 3 };
+struct TimedEvent { int cls; cudaEvent_t a, b; };
+struct Timing {
+    bool on = false;
+    std::vector<TimedEvent> ev;
+};
+// Records an event pair around one launch when timing is on (RAII).
+struct TimedLaunch {
+    Timing* t; cudaStream_t st; TimedEvent e; bool active;
+    TimedLaunch(Timing* timing, int cls, cudaStream_t s) : t(timing), st(s), active(false) {
+        if (t && t->on) {
+            e.cls = cls;
+            if (cudaEventCreate(&e.a) == cudaSuccess && cudaEventCreate(&e.b) == cudaSuccess) {
+                cudaEventRecord(e.a, st);
+                active = true;
+            }
+        }
+    }
+    ~TimedLaunch() {
+        if (active) { cudaEventRecord(e.b, st); t->ev.push_back(e); }
+    }
+};
+}  // namespace mk
+
 struct mttkrp_handle_s {
     int N;
     int64_t dims[mk::kMaxModes];
@@ -62,6 +88,7 @@ struct mttkrp_handle_s {
     int64_t bytes_held;
     int64_t remaps_done;
     int device;
+    mk::Timing* timing;       // owned; per-kernel event pairs while mttkrp_timing_begin is active
 };
 
 namespace mk {

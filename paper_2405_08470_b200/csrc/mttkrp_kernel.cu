@@ -16,6 +16,7 @@
 // are merged in shared memory by warp 0; a row that spans shards leaves one partial per shard in the
 // carry buffer and is summed, in fixed order, by k_fixup.  Rows with no nonzero are zeroed by
 // k_zero_rows from the precomputed list, so `out` is fully overwritten without a memset.
+#include <algorithm>
 #include "common.cuh"
 
 namespace mk {
@@ -253,6 +254,7 @@ static mttkrp_status_t launch_nr(const mttkrp_handle_s* h, int d, const float* c
         const int64_t groups = mm.n_empty;
         const int64_t threads = groups * (R / 4);
         const unsigned grid = (unsigned)std::min<int64_t>((threads + 255) / 256, 148 * 16);
+        TimedLaunch tl(h->timing, kClsZero, st);
         k_zero_rows<R><<<grid, 256, 0, st>>>(mm.empty_rows, mm.n_empty, out);
     }
     if (h->num_shards > 0) {
@@ -264,8 +266,14 @@ static mttkrp_status_t launch_nr(const mttkrp_handle_s* h, int d, const float* c
         for (int l = 1; l < N; ++l) a.fac[l] = factors[mm.order[l]];
         a.out = out;
         a.carry = h->carry;
-        k_mttkrp<N, R><<<(unsigned)h->num_shards, kBlockThreads, 0, st>>>(a);
-        if (mm.n_chains > 0) k_fixup<R><<<(unsigned)mm.n_chains, 128, 0, st>>>(mm.chains, h->carry, out);
+        {
+            TimedLaunch tl(h->timing, kClsMttkrp, st);
+            k_mttkrp<N, R><<<(unsigned)h->num_shards, kBlockThreads, 0, st>>>(a);
+        }
+        if (mm.n_chains > 0) {
+            TimedLaunch tl(h->timing, kClsFixup, st);
+            k_fixup<R><<<(unsigned)mm.n_chains, 128, 0, st>>>(mm.chains, h->carry, out);
+        }
     }
     MK_CUDA(cudaGetLastError());
     return MTTKRP_OK;

@@ -46,6 +46,7 @@ mttkrp_status_t launch_remap(mttkrp_handle_s* h, int from, cudaStream_t st) {
         for (int l = 0; l < N; ++l) fm.src[l] = h->mode[from].pos[h->mode[to].order[l]];
         const unsigned grid = (unsigned)((h->nnz + 255) / 256);
         const uint32_t* next = h->mode[from].next;
+        TimedLaunch tl(h->timing, kClsRemap, st);
         switch (N) {
             case 2: k_remap<2><<<grid, 256, 0, st>>>(h->rec_cur, next, h->rec_alt, h->nnz, fm); break;
             case 3: k_remap3<<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, next, (uint4*)h->rec_alt, h->nnz, fm); break;
