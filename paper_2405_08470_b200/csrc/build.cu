@@ -459,8 +459,15 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
         for (int d = 0; d < N; ++d) {
             const int e = (d + 1) % N;
             const uint32_t* perm_e = (e == 0) ? h->perm0 : h->mode[e].next;
-            k_invert<<<grid_for(nnz, 256), 256, 0, st>>>(perm_e, inv, nnz);
-            k_apply_table<<<grid_for(nnz, 256), 256, 0, st>>>(inv, h->mode[d].next, nnz);
+            if (h->remap_gather) {
+                // gather map: slot d <- inv_d[perm_e[j]] = position in layout d of element j of layout e
+                k_invert<<<grid_for(nnz, 256), 256, 0, st>>>(h->mode[d].next, inv, nnz);
+                k_gather_u32<<<grid_for(nnz, 256), 256, 0, st>>>(inv, perm_e, h->mode[d].next, nnz);
+            } else {
+                // scatter map: slot d <- inv_e[perm_d[k]] = position in layout e of element k of layout d
+                k_invert<<<grid_for(nnz, 256), 256, 0, st>>>(perm_e, inv, nnz);
+                k_apply_table<<<grid_for(nnz, 256), 256, 0, st>>>(inv, h->mode[d].next, nnz);
+            }
         }
         MK_CUDA(cudaGetLastError());
     }

@@ -88,6 +88,7 @@ struct mttkrp_handle_s {
     int64_t bytes_held;
     int64_t remaps_done;
     int device;
+    int remap_gather;         // 1: mode[d].next holds the gather map (position in layout d of element j of layout d+1)
     mk::Timing* timing;       // owned; per-kernel event pairs while mttkrp_timing_begin is active
 };
 
@@ -111,7 +112,7 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
 // ---- remap.cu -------------------------------------------------------------------------------
 mttkrp_status_t launch_remap(mttkrp_handle_s* h, int from, cudaStream_t st);   // from -> (from+1)%N, swaps copies
 mttkrp_status_t launch_export(const mttkrp_handle_s* h, int32_t* idx, float* vals, cudaStream_t st);
-mttkrp_status_t launch_perm_step(const uint32_t* next, const uint32_t* in, uint32_t* out, int64_t nnz, cudaStream_t st);
+mttkrp_status_t launch_perm_step(const uint32_t* map, int gather, const uint32_t* in, uint32_t* out, int64_t nnz, cudaStream_t st);
 
 // ---- mttkrp_kernel.cu -----------------------------------------------------------------------
 mttkrp_status_t launch_mttkrp(const mttkrp_handle_s* h, int d, const float* const* factors, int R,
