@@ -103,10 +103,6 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
     h->max_rank = max_rank;
     h->device = dev;
     h->timing = new (std::nothrow) Timing();
-    {
-        const char* env = getenv("MTTKRP_REMAP");
-        h->remap_gather = (env && strcmp(env, "scatter") == 0) ? 0 : 1;
-    }
     for (int d = 0; d < nmodes; ++d) {
         ModeMeta& mm = h->mode[d];
         choose_key_order(nmodes, dims, d, mm.order);
@@ -119,7 +115,7 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
             h->stage_out[d] = reinterpret_cast<float*>(ws + p.stage_out[d]);
         }
     }
-    h->bytes_held = (int64_t)(p.persistent_end + (size_t)(nmodes + 1) * 4 * (size_t)nnz);
+    h->bytes_held = (int64_t)(p.persistent_end + (size_t)(nmodes + 1) * 4 * (size_t)(p.num_shards * p.shard_nnz));
     mttkrp_status_t s = build_format(h, p, ws, idx, vals, static_cast<cudaStream_t>(cuda_stream));
     if (s != MTTKRP_OK) { delete h->timing; delete h; return s; }
     *out = h;
@@ -260,7 +256,7 @@ mttkrp_status_t mttkrp_get_perm(mttkrp_handle_t h, int d, uint32_t* perm_dev, ui
     uint32_t* b = (d % 2 == 0) ? scratch_dev : perm_dev;
     MK_CUDA(cudaMemcpyAsync(a, h->perm0, (size_t)h->nnz * 4, cudaMemcpyDeviceToDevice, st));
     for (int j = 0; j < d; ++j) {
-        MK_TRY(launch_perm_step(h->mode[j].next, h->remap_gather, a, b, h->nnz, st));
+        MK_TRY(launch_perm_step(h->mode[j].next, a, b, h->nnz, st));
         uint32_t* t = a; a = b; b = t;
     }
     return MTTKRP_OK;

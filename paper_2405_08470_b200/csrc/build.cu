@@ -33,9 +33,10 @@ static int choose_shard_nnz(int64_t nnz) {
 mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_rank, WorkspacePlan* p) {
     memset(p, 0, sizeof(*p));
     const size_t n = (size_t)nnz;
-    const size_t rec_bytes = (size_t)(N + 1) * 4 * n;
     p->shard_nnz = choose_shard_nnz(nnz);
     p->num_shards = (nnz + p->shard_nnz - 1) / p->shard_nnz;
+    // both tensor copies are padded to a whole number of shards (zero-valued copies of the last nonzero)
+    const size_t rec_bytes = (size_t)(N + 1) * 4 * (size_t)(p->num_shards * p->shard_nnz);
     size_t off = 0;
     p->rec_a = off; off = align_up(off + rec_bytes);
     for (int d = 0; d < N; ++d) { p->next[d] = off; off = align_up(off + 4 * n); }
@@ -267,15 +268,16 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_scatter(const uint32_t* 
 // rec[k] = { idx[order[0]][perm[k]], ..., idx[order[N-1]][perm[k]], val[perm[k]] }
 struct OrderArg { int v[kMaxModes]; };
 
+// Positions k in [nnz, nnz_pad) are padding: the keys of the last nonzero with value 0.
 __global__ void k_build_records(const int32_t* __restrict__ idx, const float* __restrict__ vals,
-                                const uint32_t* __restrict__ perm, int64_t nnz, int N, OrderArg order,
+                                const uint32_t* __restrict__ perm, int64_t nnz, int64_t nnz_pad, int N, OrderArg order,
                                 uint32_t* __restrict__ rec) {
     int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= nnz) return;
-    uint32_t src = perm[k];
+    if (k >= nnz_pad) return;
+    uint32_t src = perm[k < nnz ? k : nnz - 1];
     uint32_t* r = rec + (size_t)k * (N + 1);
     for (int l = 0; l < N; ++l) r[l] = (uint32_t)idx[(size_t)order.v[l] * nnz + src];
-    r[N] = __float_as_uint(vals[src]);
+    r[N] = k < nnz ? __float_as_uint(vals[src]) : 0u;
 }
 
 __global__ void k_mark_rows(const uint32_t* __restrict__ kd, int64_t nnz, uint32_t* __restrict__ present) {
@@ -452,22 +454,17 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
         // tensor copy in mode-0 order
         OrderArg oa;
         for (int l = 0; l < kMaxModes; ++l) oa.v[l] = h->mode[0].order[l];
-        k_build_records<<<grid_for(nnz, 256), 256, 0, st>>>(idx, vals, h->perm0, nnz, N, oa, h->rec_cur);
-        // next_d[k] = inv_{d+1}[perm_d[k]]; slot d still holds perm_d; go d = 0..N-1, the last one
-        // needs perm_0 which slot 0 no longer holds -> use the perm0 copy.
+        const int64_t nnz_pad = nshards * (int64_t)S;
+        k_build_records<<<grid_for(nnz_pad, 256), 256, 0, st>>>(idx, vals, h->perm0, nnz, nnz_pad, N, oa, h->rec_cur);
+        // Slot d still holds perm_d; go d = 0..N-1, the last one needs perm_0, which slot 0 no longer
+        // holds -> use the perm0 copy.
         uint32_t* inv = keyA;
         for (int d = 0; d < N; ++d) {
             const int e = (d + 1) % N;
             const uint32_t* perm_e = (e == 0) ? h->perm0 : h->mode[e].next;
-            if (h->remap_gather) {
-                // gather map: slot d <- inv_d[perm_e[j]] = position in layout d of element j of layout e
-                k_invert<<<grid_for(nnz, 256), 256, 0, st>>>(h->mode[d].next, inv, nnz);
-                k_gather_u32<<<grid_for(nnz, 256), 256, 0, st>>>(inv, perm_e, h->mode[d].next, nnz);
-            } else {
-                // scatter map: slot d <- inv_e[perm_d[k]] = position in layout e of element k of layout d
-                k_invert<<<grid_for(nnz, 256), 256, 0, st>>>(perm_e, inv, nnz);
-                k_apply_table<<<grid_for(nnz, 256), 256, 0, st>>>(inv, h->mode[d].next, nnz);
-            }
+            // gather map: slot d <- inv_d[perm_e[j]] = position in layout d of element j of layout e
+            k_invert<<<grid_for(nnz, 256), 256, 0, st>>>(h->mode[d].next, inv, nnz);
+            k_gather_u32<<<grid_for(nnz, 256), 256, 0, st>>>(inv, perm_e, h->mode[d].next, nnz);
         }
         MK_CUDA(cudaGetLastError());
     }

@@ -35,7 +35,8 @@ void set_error(const char* fmt, ...);
 struct ModeMeta {
     int order[kMaxModes];     // sort-key order of this layout, order[0] == mode
     int pos[kMaxModes];       // pos[m] = level of mode m in `order`
-    uint32_t* next;           // [nnz] position in layout (d+1)%N of the element at position k here
+    uint32_t* next;           // [nnz] gather map of the remap d -> (d+1)%N: position in THIS layout of the
+                              // element at position j of the next layout (the paper's remap id, read backwards)
     uint32_t* empty_rows;     // [n_empty] output rows without a nonzero
     int64_t n_empty;
     uint32_t* chains;         // [n_chains][3] = {first shard, last shard, row} for rows spanning shards
@@ -88,7 +89,6 @@ struct mttkrp_handle_s {
     int64_t bytes_held;
     int64_t remaps_done;
     int device;
-    int remap_gather;         // 1: mode[d].next holds the gather map (position in layout d of element j of layout d+1)
     mk::Timing* timing;       // owned; per-kernel event pairs while mttkrp_timing_begin is active
 };
 
@@ -112,7 +112,7 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
 // ---- remap.cu -------------------------------------------------------------------------------
 mttkrp_status_t launch_remap(mttkrp_handle_s* h, int from, cudaStream_t st);   // from -> (from+1)%N, swaps copies
 mttkrp_status_t launch_export(const mttkrp_handle_s* h, int32_t* idx, float* vals, cudaStream_t st);
-mttkrp_status_t launch_perm_step(const uint32_t* map, int gather, const uint32_t* in, uint32_t* out, int64_t nnz, cudaStream_t st);
+mttkrp_status_t launch_perm_step(const uint32_t* map, const uint32_t* in, uint32_t* out, int64_t nnz, cudaStream_t st);
 
 // ---- mttkrp_kernel.cu -----------------------------------------------------------------------
 mttkrp_status_t launch_mttkrp(const mttkrp_handle_s* h, int d, const float* const* factors, int R,

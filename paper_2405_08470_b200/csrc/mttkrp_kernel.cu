@@ -1,21 +1,29 @@
 // spMTTKRP for one mode on the mode-d layout (Alg. 2 "Elementwise Computation", PAPER.md:197-217;
 // Alg. 4 thread-block mapping, as function only; the mapping here is this
-// library's own).
+// library's own, made for sm_100a).
 //
 // Layout: records sorted by the key tuple (k_0 = i_d, k_1, ..., k_{N-1}); record = N int32 keys in
 // that order + fp32 value.  A thread block owns one shard = shard_nnz consecutive records
-// (equal-nnz shards).  Inside the block a GROUP of R/4 lanes (one float4 of the rank dimension per
-// lane) walks a contiguous chunk of the shard one nonzero at a time:
+// (equal-nnz shards).  Inside the block a GROUP of R/V lanes (V = 8 rank columns per lane, one
+// 256-bit LDG per factor row per lane) walks a contiguous chunk of the shard one nonzero at a time:
 //   l(r) = val * prod_w A_w[i_w, r]         (Alg. 2 lines 8-13)
 //   Y_d[i_d, r] += l(r)                     (Alg. 2 lines 14-15)
 // Because the chunk is sorted, the products are nested sums (a CSF-style factoring of the same
 // expression):  Y[k_0] = sum_{k_1} A[k_1] * ( sum_{k_2} A[k_2] * ( ... sum_{k_{N-1}} val * A[k_{N-1}] ) ),
-// so a factor row is gathered once per run of equal key prefix rather than once per nonzero.
+// so the row of level l is gathered once per run of equal (k_0..k_l), at the END of the run.
+//
+// Pipeline per warp: records are staged into a shared-memory ring with cp.async (4 stages of 4
+// records per group, interleaved by group so one LDS.128 serves all groups without bank conflicts);
+// two steps ahead of the arithmetic the group reads record j and j+1 from the ring, derives the
+// end-of-run flags, and issues the factor-row gathers for step j into rotating registers.
+// The arithmetic is packed fp32x2 FMA (FFMA2).
+//
 // Rows that begin and end inside a chunk are stored with plain stores by their only owner
 // (Observation 2: no global atomics).  The first/last partial rows of each chunk
-// are merged in shared memory by warp 0; a row that spans shards leaves one partial per shard in the
-// carry buffer and is summed, in fixed order, by k_fixup.  Rows with no nonzero are zeroed by
-// k_zero_rows from the precomputed list, so `out` is fully overwritten without a memset.
+// are merged in shared memory, first per warp, then per block; a row that spans shards leaves one
+// partial per shard in the carry buffer and is summed, in fixed order, by k_fixup.  Rows with no
+// nonzero are zeroed by k_zero_rows from the precomputed list, so `out` is fully overwritten
+// without a memset.
 #include <algorithm>
 #include "common.cuh"
 
@@ -23,28 +31,132 @@ namespace mk {
 
 template <int N>
 struct KernelArgs {
-    const uint32_t* rec;
-    int64_t nnz;
+    const uint32_t* rec;     // padded to num_shards * shard_nnz records
+    int64_t nnz;             // padded record count
     int shard_nnz;
     const float* fac[N];     // fac[l] = factor of the mode at key level l (fac[0] unused)
     float* out;
     float* carry;            // [2*num_shards][R]
 };
 
-__device__ __forceinline__ float4 ld_row(const float* __restrict__ A, uint32_t row, int R, int sub) {
-    return __ldg(reinterpret_cast<const float4*>(A + (size_t)row * R) + sub);
+// ---- small PTX helpers ------------------------------------------------------------------------
+__device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c) {
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;"
+        : "=l"(d)
+        : "l"(*reinterpret_cast<unsigned long long*>(&a)), "l"(*reinterpret_cast<unsigned long long*>(&b)),
+          "l"(*reinterpret_cast<unsigned long long*>(&c)));
+    return *reinterpret_cast<float2*>(&d);
 }
-__device__ __forceinline__ void fma4(float4& acc, const float4& a, const float4& b) {
-    acc.x = fmaf(a.x, b.x, acc.x);
-    acc.y = fmaf(a.y, b.y, acc.y);
-    acc.z = fmaf(a.z, b.z, acc.z);
-    acc.w = fmaf(a.w, b.w, acc.w);
+__device__ __forceinline__ float2 splat2(float s) {
+    unsigned long long d;
+    asm("mov.b64 %0, {%1, %1};" : "=l"(d) : "f"(s));
+    return *reinterpret_cast<float2*>(&d);
 }
-__device__ __forceinline__ void fma4s(float4& acc, float s, const float4& b) {
-    acc.x = fmaf(s, b.x, acc.x);
-    acc.y = fmaf(s, b.y, acc.y);
-    acc.z = fmaf(s, b.z, acc.z);
-    acc.w = fmaf(s, b.w, acc.w);
+
+template <int V>
+struct Vec {                 // V rank columns of one lane, as fp32 pairs
+    float2 p[V / 2];
+};
+
+template <int V>
+__device__ __forceinline__ Vec<V> vzero() {
+    Vec<V> r;
+#pragma unroll
+    for (int i = 0; i < V / 2; ++i) r.p[i] = make_float2(0.f, 0.f);
+    return r;
+}
+
+// One lane's V columns of factor row `row` (read-only path; 256-bit or 128-bit load).
+template <int V>
+__device__ __forceinline__ Vec<V> ld_row(const float* __restrict__ A, uint32_t row, int R, int sub) {
+    const float* p = A + (size_t)row * R + sub * V;
+    Vec<V> r;
+    if constexpr (V == 8) {
+        asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                     : "=f"(r.p[0].x), "=f"(r.p[0].y), "=f"(r.p[1].x), "=f"(r.p[1].y), "=f"(r.p[2].x), "=f"(r.p[2].y),
+                       "=f"(r.p[3].x), "=f"(r.p[3].y)
+                     : "l"(p));
+    } else {
+        float4 v = __ldg(reinterpret_cast<const float4*>(p));
+        r.p[0] = make_float2(v.x, v.y);
+        r.p[1] = make_float2(v.z, v.w);
+    }
+    return r;
+}
+// acc += a * b (elementwise), acc += s * b
+template <int V>
+__device__ __forceinline__ void vfma(Vec<V>& acc, const Vec<V>& a, const Vec<V>& b) {
+#pragma unroll
+    for (int i = 0; i < V / 2; ++i) acc.p[i] = ffma2(a.p[i], b.p[i], acc.p[i]);
+}
+template <int V>
+__device__ __forceinline__ void vfmas(Vec<V>& acc, float s, const Vec<V>& b) {
+    const float2 ss = splat2(s);
+#pragma unroll
+    for (int i = 0; i < V / 2; ++i) acc.p[i] = ffma2(ss, b.p[i], acc.p[i]);
+}
+template <int V>
+__device__ __forceinline__ void vstore(float* dst, const Vec<V>& v) {
+#pragma unroll
+    for (int i = 0; i < V / 4; ++i)
+        *reinterpret_cast<float4*>(dst + 4 * i) = make_float4(v.p[2 * i].x, v.p[2 * i].y, v.p[2 * i + 1].x, v.p[2 * i + 1].y);
+}
+
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, bool pred) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(pred ? 16 : 0) : "memory");
+}
+__device__ __forceinline__ void cp_async4(uint32_t dst, const void* src, bool pred) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(dst), "l"(src), "r"(pred ? 4 : 0) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int NPEND>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(NPEND) : "memory"); }
+
+// ---- compile-time geometry ---------------------------------------------------------------------
+template <int N, int R>
+struct Geo {
+    static constexpr int V = (R >= 16) ? 8 : 4;          // rank columns per lane
+    static constexpr int LPN = R / V;                    // lanes per nonzero (group size)
+    static constexpr int NPW = 32 / LPN;                 // groups per warp
+    static constexpr int WARPS = kBlockThreads / 32;
+    static constexpr int G = WARPS * NPW;                // groups per block
+    static constexpr int K = 4;                          // records per group per ring stage
+    static constexpr int STAGES = 4;
+    static constexpr int RECW = N + 1;                   // record words
+    static constexpr int SLOTW = (RECW + 3) / 4 * 4;     // ring slot words (16-byte multiple)
+    static constexpr int RING_WORDS = STAGES * K * NPW * SLOTW;        // per warp
+    static constexpr int ENT_WORDS = 2 * NPW * R;                       // per warp: first/last partial rows
+    static constexpr int WARP_WORDS = RING_WORDS > ENT_WORDS ? RING_WORDS : ENT_WORDS;
+    static constexpr int NL = N - 1;                     // accumulator levels t[0..NL-1]
+    static constexpr int SMEM_BYTES = 4 * (WARPS * WARP_WORDS + WARPS * NPW * R + 2 * WARPS * R + WARPS * 2 * NPW + 2 * WARPS);
+};
+
+// Sequential merge of partial rows (rows[e] < 0 = unused).  Runs of equal row id are adjacent.
+// emit(row, acc, is_first_run, is_last_run): lane c holds columns c, c+32.
+template <int R, class Emit>
+__device__ __forceinline__ void merge_runs(const int* rows, const float* vecs, int n, int lane, Emit emit) {
+    constexpr int CPL = (R + 31) / 32;
+    float acc[CPL];
+#pragma unroll
+    for (int j = 0; j < CPL; ++j) acc[j] = 0.f;
+    int cur_row = -1, run = 0;
+    for (int e = 0; e < n; ++e) {
+        const int r = rows[e];
+        if (r < 0) continue;
+        if (r != cur_row) {
+            if (cur_row >= 0) { emit(cur_row, acc, run == 0, false); ++run; }
+            cur_row = r;
+#pragma unroll
+            for (int j = 0; j < CPL; ++j) acc[j] = 0.f;
+        }
+#pragma unroll
+        for (int j = 0; j < CPL; ++j) {
+            const int col = lane + 32 * j;
+            if (col < R) acc[j] += vecs[(size_t)e * R + col];
+        }
+    }
+    if (cur_row >= 0) emit(cur_row, acc, run == 0, true);
 }
 
 template <int N>
@@ -53,159 +165,222 @@ struct Rec {
     float val;
 };
 
-template <int N>
-__device__ __forceinline__ Rec<N> load_rec(const uint32_t* __restrict__ rec, int64_t pos) {
-    Rec<N> r;
-    const uint32_t* p = rec + (size_t)pos * (N + 1);
-    if constexpr (N == 3) {
-        uint4 v = __ldg(reinterpret_cast<const uint4*>(p));
-        r.k[0] = v.x; r.k[1] = v.y; r.k[2] = v.z; r.val = __uint_as_float(v.w);
-    } else if constexpr (N == 7) {
-        uint4 a = __ldg(reinterpret_cast<const uint4*>(p));
-        uint4 b = __ldg(reinterpret_cast<const uint4*>(p) + 1);
-        r.k[0] = a.x; r.k[1] = a.y; r.k[2] = a.z; r.k[3] = a.w;
-        r.k[4] = b.x; r.k[5] = b.y; r.k[6] = b.z; r.val = __uint_as_float(b.w);
-    } else if constexpr ((N + 1) % 2 == 0) {
-        uint32_t w[N + 1];
-#pragma unroll
-        for (int j = 0; j < (N + 1) / 2; ++j) {
-            uint2 v = __ldg(reinterpret_cast<const uint2*>(p) + j);
-            w[2 * j] = v.x; w[2 * j + 1] = v.y;
-        }
-#pragma unroll
-        for (int j = 0; j < N; ++j) r.k[j] = w[j];
-        r.val = __uint_as_float(w[N]);
-    } else {
-#pragma unroll
-        for (int j = 0; j < N; ++j) r.k[j] = __ldg(p + j);
-        r.val = __uint_as_float(__ldg(p + N));
-    }
-    return r;
-}
-
 template <int N, int R>
 __global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a) {
-    constexpr int LPN = R / 4;                   // lanes per nonzero
-    constexpr int NPW = 32 / LPN;                // groups per warp
-    constexpr int G = (kBlockThreads / 32) * NPW;   // groups per block
-    constexpr int NL = N - 1;                    // accumulator levels t[0..NL-1]
-    __shared__ __align__(16) float ent_vec[2 * G][R];
-    __shared__ int ent_row[2 * G];
+    using Ge = Geo<N, R>;
+    constexpr int V = Ge::V, LPN = Ge::LPN, NPW = Ge::NPW, WARPS = Ge::WARPS, G = Ge::G, K = Ge::K;
+    constexpr int STAGES = Ge::STAGES, RECW = Ge::RECW, SLOTW = Ge::SLOTW, NL = Ge::NL;
+    constexpr int ROWW = NPW * SLOTW;                     // ring words between consecutive records of a group
+    constexpr int STAGEW = K * ROWW;                      // ring words per stage
+    constexpr bool PIECE16 = (RECW % 4 == 0);             // 16-byte cp.async pieces, else 4-byte
+    constexpr int PW = PIECE16 ? 4 : 1;                   // piece words
+    constexpr int PPR = RECW / PW;                        // pieces per record
+    constexpr int NPIECE = (K * PPR + LPN - 1) / LPN;     // pieces per lane per round
+    static_assert(K == 4 && STAGES == 4, "the step schedule below is written for 4 stages of 4 records");
+
+    extern __shared__ uint4 smem_raw[];
+    // carve-up (Geo::SMEM_BYTES): record rings (later the groups' last partial rows) | the groups'
+    // first partial rows | the warps' first/last partial rows | row ids
+    uint32_t (*s_warp)[Ge::WARP_WORDS] = reinterpret_cast<uint32_t (*)[Ge::WARP_WORDS]>(smem_raw);
+    float (*s_first)[NPW][R] = reinterpret_cast<float (*)[NPW][R]>(&s_warp[WARPS][0]);
+    float (*s_wvec)[R] = reinterpret_cast<float (*)[R]>(&s_first[WARPS][0][0]);
+    int (*s_erow)[2 * NPW] = reinterpret_cast<int (*)[2 * NPW]>(&s_wvec[2 * WARPS][0]);
+    int* s_wrow = &s_erow[WARPS][0];
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int gi = warp * NPW + lane / LPN;
-    const int sub = lane % LPN;
+    const int g = lane / LPN, sub = lane % LPN;
     const int64_t shard = blockIdx.x;
+    // The record array is padded to a whole number of shards (value 0, keys of the last nonzero),
+    // so every chunk holds exactly C records and the loop needs no bounds checks.
     const int64_t s_begin = shard * (int64_t)a.shard_nnz;
-    const int64_t s_end = min(s_begin + a.shard_nnz, a.nnz);
-    const int C = a.shard_nnz / G;
-    const int64_t c_begin = min(s_begin + (int64_t)gi * C, s_end);
-    const int64_t c_end = min(c_begin + C, s_end);
+    const int64_t s_end = s_begin + a.shard_nnz;
+    const int C = a.shard_nnz / G;                        // records per group; a multiple of K
+    const int nrounds = C / K;
+    const uint32_t* const grec = a.rec + (size_t)(s_begin + (int64_t)(warp * NPW + g) * C) * RECW;
 
-    uint32_t key[NL];
-    float4 t[NL];
-    float4 rowv[NL];                             // rowv[l] = A_{level l}[key[l]] for l >= 1
-#pragma unroll
-    for (int l = 0; l < NL; ++l) {
-        key[l] = 0xffffffffu;
-        t[l] = make_float4(0.f, 0.f, 0.f, 0.f);
-        rowv[l] = make_float4(0.f, 0.f, 0.f, 0.f);
-    }
-    int seg = 0;                                 // output-row segments finished so far in this chunk
-    float* const entF = &ent_vec[2 * gi][sub * 4];
-    float* const entL = &ent_vec[2 * gi + 1][sub * 4];
+    uint32_t* const ring = &s_warp[warp][0];
+    const uint32_t* const ring_g = ring + g * SLOTW;      // this group's column of the ring
+    const uint32_t ring_gs = (uint32_t)__cvta_generic_to_shared(ring_g);
 
-    if (c_begin < c_end) {
-        Rec<N> cur = load_rec<N>(a.rec, c_begin);
-        for (int64_t pos = c_begin; pos < c_end; ++pos) {
-            Rec<N> nxt = cur;
-            if (pos + 1 < c_end) nxt = load_rec<N>(a.rec, pos + 1);
-            const float4 alast = ld_row(a.fac[N - 1], cur.k[N - 1], R, sub);
-            int c = NL;                          // first key level that differs from the running prefix
+    auto issue_round = [&](int r) {
+        if (r < nrounds) {
+            const uint32_t* src = grec + (size_t)r * (K * RECW);
+            const uint32_t dst = ring_gs + 4u * (uint32_t)((r & (STAGES - 1)) * STAGEW);
 #pragma unroll
-            for (int l = NL - 1; l >= 0; --l)
-                if (cur.k[l] != key[l]) c = l;
-            if (c < NL) {
-                // close the finished runs, innermost first: t[l-1] += A[key[l]] * t[l]
-#pragma unroll
-                for (int l = NL - 1; l >= 1; --l) {
-                    if (l >= c) {
-                        fma4(t[l - 1], rowv[l], t[l]);
-                        t[l] = make_float4(0.f, 0.f, 0.f, 0.f);
-                    }
-                }
-                if (c == 0) {
-                    if (key[0] != 0xffffffffu) {
-                        float* dst = (seg == 0) ? entF : a.out + (size_t)key[0] * R + sub * 4;
-                        *reinterpret_cast<float4*>(dst) = t[0];
-                        if (seg == 0 && sub == 0) ent_row[2 * gi] = (int)key[0];
-                        ++seg;
-                    }
-                    t[0] = make_float4(0.f, 0.f, 0.f, 0.f);
-                }
-#pragma unroll
-                for (int l = 0; l < NL; ++l) {
-                    if (l >= c) {
-                        key[l] = cur.k[l];
-                        if (l >= 1) rowv[l] = ld_row(a.fac[l], key[l], R, sub);
-                    }
+            for (int i = 0; i < NPIECE; ++i) {
+                const int p = sub + i * LPN;
+                if (p < K * PPR) {
+                    const int jj = p / PPR, q = p % PPR;
+                    if constexpr (PIECE16) cp_async16(dst + 4u * (uint32_t)(jj * ROWW + q * PW), src + jj * RECW + q * PW, true);
+                    else cp_async4(dst + 4u * (uint32_t)(jj * ROWW + q * PW), src + jj * RECW + q * PW, true);
                 }
             }
-            fma4s(t[NL - 1], cur.val, alast);
-            cur = nxt;
+        }
+        cp_async_commit();
+    };
+    auto read_rec = [&](const uint32_t* slot) {
+        Rec<N> r;
+        uint32_t w[SLOTW];
+        const uint4* p = reinterpret_cast<const uint4*>(slot);
+#pragma unroll
+        for (int i = 0; i < SLOTW / 4; ++i) {
+            const uint4 v = p[i];
+            w[4 * i] = v.x; w[4 * i + 1] = v.y; w[4 * i + 2] = v.z; w[4 * i + 3] = v.w;
         }
 #pragma unroll
-        for (int l = NL - 1; l >= 1; --l) fma4(t[l - 1], rowv[l], t[l]);
-        float* dst = (seg == 0) ? entF : entL;
-        *reinterpret_cast<float4*>(dst) = t[0];
-        if (sub == 0) {
-            ent_row[2 * gi + (seg == 0 ? 0 : 1)] = (int)key[0];
-            if (seg == 0) ent_row[2 * gi + 1] = -1;
+        for (int i = 0; i < N; ++i) r.k[i] = w[i];
+        r.val = __uint_as_float(w[N]);
+        return r;
+    };
+
+    Vec<V> t[NL];                                         // t[0] = output row accumulator
+#pragma unroll
+    for (int l = 0; l < NL; ++l) t[l] = vzero<V>();
+    Vec<V> al[2];                                         // last-level rows for the two steps in flight
+    Vec<V> rb[NL][2];                                     // rb[l][slot]: row of level l, gathered at the end of its run
+    float val[2] = {0.f, 0.f};
+    unsigned ef[2] = {0u, 0u};                            // bit l: the run of level l ends at this step
+    Rec<N> cur;
+    int seg = 0;                                          // output-row segments finished in this chunk
+
+    // Prepare step j (record `cur`; `nslot` holds record j+1): end-of-run flags and the row gathers.
+    auto lookahead = [&](int j, const uint32_t* nslot, int slot) {
+        const Rec<N> nxt = read_rec(nslot);               // stale past the chunk end; masked by `last`
+        unsigned e = 0u;
+        bool diff = (j + 1 >= C);
+#pragma unroll
+        for (int l = 0; l < NL; ++l) {
+            diff = diff || (nxt.k[l] != cur.k[l]);
+            e |= diff ? (1u << l) : 0u;
         }
-    } else if (sub == 0) {
-        ent_row[2 * gi] = -1;
-        ent_row[2 * gi + 1] = -1;
+        al[slot] = ld_row<V>(a.fac[N - 1], cur.k[N - 1], R, sub);
+#pragma unroll
+        for (int l = 1; l < NL; ++l)
+            if (e & (1u << l)) rb[l][slot] = ld_row<V>(a.fac[l], cur.k[l], R, sub);
+        val[slot] = cur.val;
+        ef[slot] = e;
+        cur = nxt;
+    };
+    // Arithmetic of step j (its record sits at `jslot`).
+    auto process = [&](int j, const uint32_t* jslot, int slot) {
+        const unsigned e = ef[slot];
+        vfmas<V>(t[NL - 1], val[slot], al[slot]);
+#pragma unroll
+        for (int l = NL - 1; l >= 1; --l) {
+            if (e & (1u << l)) {
+                vfma<V>(t[l - 1], rb[l][slot], t[l]);
+                t[l] = vzero<V>();
+            }
+        }
+        if ((e & 1u) && j + 1 < C) {                      // an output row ends inside the chunk
+            const uint32_t row = jslot[0];
+            float* dst = (seg == 0) ? &s_first[warp][g][sub * V] : a.out + (size_t)row * R + sub * V;
+            vstore<V>(dst, t[0]);
+            if (seg == 0 && sub == 0) s_erow[warp][2 * g] = (int)row;
+            ++seg;
+            t[0] = vzero<V>();
+        }
+    };
+
+#pragma unroll
+    for (int r = 0; r < STAGES - 1; ++r) issue_round(r);
+    cp_async_wait<STAGES - 2>();                          // round 0 has landed
+    __syncwarp();
+    cur = read_rec(ring_g);
+    lookahead(0, ring_g + 1 * ROWW, 0);
+    lookahead(1, ring_g + 2 * ROWW, 1);
+    for (int r = 0; r < nrounds; ++r) {
+        issue_round(r + STAGES - 1);
+        cp_async_wait<STAGES - 2>();                      // rounds <= r+1 have landed
+        __syncwarp();
+        const uint32_t* cs = ring_g + (r & (STAGES - 1)) * STAGEW;          // this round's stage
+        const uint32_t* ns = ring_g + ((r + 1) & (STAGES - 1)) * STAGEW;    // next round's stage
+        const int j0 = r * K;
+        const bool more = r + 1 < nrounds;
+        process(j0 + 0, cs + 0 * ROWW, 0);
+        lookahead(j0 + 2, cs + 3 * ROWW, 0);
+        process(j0 + 1, cs + 1 * ROWW, 1);
+        lookahead(j0 + 3, ns + 0 * ROWW, 1);
+        process(j0 + 2, cs + 2 * ROWW, 0);
+        if (more) lookahead(j0 + 4, ns + 1 * ROWW, 0);
+        process(j0 + 3, cs + 3 * ROWW, 1);
+        if (more) lookahead(j0 + 5, ns + 2 * ROWW, 1);
+        __syncwarp();                                     // everyone is done with round r's stage
+    }
+    cp_async_wait<0>();
+    const uint32_t last_row = ring_g[((C - 1) & (STAGES * K - 1)) * ROWW];
+    __syncwarp();
+    // chunk epilogue: the still-open row goes to the first (seg == 0) or last partial-row entry
+    float* const s_last = reinterpret_cast<float*>(ring);               // [NPW][R], aliases the ring
+    {
+        float* dst = (seg == 0) ? &s_first[warp][g][sub * V] : s_last + g * R + sub * V;
+        vstore<V>(dst, t[0]);
+        if (sub == 0) {
+            s_erow[warp][2 * g + (seg == 0 ? 0 : 1)] = (int)last_row;
+            if (seg == 0) s_erow[warp][2 * g + 1] = -1;
+        }
+    }
+    if (lane == 0) { s_wrow[2 * warp] = -1; s_wrow[2 * warp + 1] = -1; }
+    __syncwarp();
+
+    // level 1: merge this warp's 2*NPW partial rows; interior rows are complete -> plain stores
+    {
+        const float* firsts = &s_first[warp][0][0];
+        constexpr int CPL = (R + 31) / 32;
+        float acc[CPL];
+#pragma unroll
+        for (int q = 0; q < CPL; ++q) acc[q] = 0.f;
+        int cur_row = -1, run = 0;
+        auto emit = [&](int row, bool is_last) {
+            float* dst;
+            if (run == 0) { dst = &s_wvec[2 * warp][0]; if (lane == 0) s_wrow[2 * warp] = row; }
+            else if (is_last) { dst = &s_wvec[2 * warp + 1][0]; if (lane == 0) s_wrow[2 * warp + 1] = row; }
+            else dst = a.out + (size_t)row * R;
+#pragma unroll
+            for (int q = 0; q < CPL; ++q) {
+                const int col = lane + 32 * q;
+                if (col < R) dst[col] = acc[q];
+            }
+            ++run;
+        };
+        for (int e = 0; e < 2 * NPW; ++e) {
+            const int r = s_erow[warp][e];
+            if (r < 0) continue;
+            if (r != cur_row) {
+                if (cur_row >= 0) emit(cur_row, false);
+                cur_row = r;
+#pragma unroll
+                for (int q = 0; q < CPL; ++q) acc[q] = 0.f;
+            }
+            const float* v = (e & 1) ? s_last + (e >> 1) * R : firsts + (e >> 1) * R;
+#pragma unroll
+            for (int q = 0; q < CPL; ++q) {
+                const int col = lane + 32 * q;
+                if (col < R) acc[q] += v[col];
+            }
+        }
+        if (cur_row >= 0) emit(cur_row, true);
     }
     __syncthreads();
 
-    // Merge the chunk-boundary partials in order; runs of equal row are adjacent.
-    if (warp == 0 && s_begin < s_end) {
-        const uint32_t first_row = __ldg(a.rec + (size_t)s_begin * (N + 1));
-        const uint32_t last_row = __ldg(a.rec + (size_t)(s_end - 1) * (N + 1));
-        const bool head_shared = s_begin > 0 && __ldg(a.rec + (size_t)(s_begin - 1) * (N + 1)) == first_row;
-        const bool tail_shared = s_end < a.nnz && __ldg(a.rec + (size_t)s_end * (N + 1)) == last_row;
-        constexpr int CPL = (R + 31) / 32;       // columns per lane
-        float acc[CPL];
-#pragma unroll
-        for (int j = 0; j < CPL; ++j) acc[j] = 0.f;
-        int cur_row = -1;
-        auto emit = [&](int row) {
+    // level 2: merge the warps' partial rows; rows shared with a neighbouring shard go to the carry buffer
+    if (warp == 0) {
+        const uint32_t first_row = __ldg(a.rec + (size_t)s_begin * RECW);
+        const uint32_t end_row = __ldg(a.rec + (size_t)(s_end - 1) * RECW);
+        const bool head_shared = s_begin > 0 && __ldg(a.rec + (size_t)(s_begin - 1) * RECW) == first_row;
+        const bool tail_shared = s_end < a.nnz && __ldg(a.rec + (size_t)s_end * RECW) == end_row;
+        constexpr int CPL = (R + 31) / 32;
+        merge_runs<R>(s_wrow, &s_wvec[0][0], 2 * WARPS, lane, [&](int row, const float* acc, bool, bool) {
             float* dst;
             if ((uint32_t)row == first_row && head_shared) dst = a.carry + (size_t)(2 * shard) * R;
-            else if ((uint32_t)row == last_row && tail_shared) dst = a.carry + (size_t)(2 * shard + 1) * R;
+            else if ((uint32_t)row == end_row && tail_shared) dst = a.carry + (size_t)(2 * shard + 1) * R;
             else dst = a.out + (size_t)row * R;
 #pragma unroll
-            for (int j = 0; j < CPL; ++j) {
-                int col = lane + 32 * j;
-                if (col < R) dst[col] = acc[j];
+            for (int q = 0; q < CPL; ++q) {
+                const int col = lane + 32 * q;
+                if (col < R) dst[col] = acc[q];
             }
-        };
-        for (int e = 0; e < 2 * G; ++e) {
-            const int r = ent_row[e];
-            if (r < 0) continue;
-            if (r != cur_row) {
-                if (cur_row >= 0) emit(cur_row);
-                cur_row = r;
-#pragma unroll
-                for (int j = 0; j < CPL; ++j) acc[j] = 0.f;
-            }
-#pragma unroll
-            for (int j = 0; j < CPL; ++j) {
-                int col = lane + 32 * j;
-                if (col < R) acc[j] += ent_vec[e][col];
-            }
-        }
-        if (cur_row >= 0) emit(cur_row);
+        });
     }
 }
 
@@ -260,15 +435,21 @@ static mttkrp_status_t launch_nr(const mttkrp_handle_s* h, int d, const float* c
     if (h->num_shards > 0) {
         KernelArgs<N> a;
         a.rec = h->rec_cur;
-        a.nnz = h->nnz;
+        a.nnz = h->num_shards * (int64_t)h->shard_nnz;
         a.shard_nnz = h->shard_nnz;
         a.fac[0] = nullptr;
         for (int l = 1; l < N; ++l) a.fac[l] = factors[mm.order[l]];
         a.out = out;
         a.carry = h->carry;
         {
+            constexpr int smem = Geo<N, R>::SMEM_BYTES;
+            static bool attr_set = false;
+            if (!attr_set) {
+                MK_CUDA(cudaFuncSetAttribute(k_mttkrp<N, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+                attr_set = true;
+            }
             TimedLaunch tl(h->timing, kClsMttkrp, st);
-            k_mttkrp<N, R><<<(unsigned)h->num_shards, kBlockThreads, 0, st>>>(a);
+            k_mttkrp<N, R><<<(unsigned)h->num_shards, kBlockThreads, smem, st>>>(a);
         }
         if (mm.n_chains > 0) {
             TimedLaunch tl(h->timing, kClsFixup, st);
