@@ -3,6 +3,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include "common.cuh"
@@ -44,6 +45,18 @@ static int ceil_log2(int64_t x) {
 static mttkrp_status_t ensure_layout(mttkrp_handle_s* h, int d, cudaStream_t st) {
     while (h->cur != d) MK_TRY(launch_remap(h, h->cur, st));
     return MTTKRP_OK;
+}
+
+// Mode d on whatever layout is resident: separate remap passes until the copy is one step before
+// d, then the last step fused into the MTTKRP kernel (Alg. 4); the cyclic order
+// of Alg. 5 therefore runs one kernel per mode.
+static mttkrp_status_t run_mode(mttkrp_handle_s* h, int d, const float* const* factors, int R, float* out, cudaStream_t st) {
+    if (h->cur == d || !h->fuse || h->nnz == 0) {
+        MK_TRY(ensure_layout(h, d, st));
+        return launch_mttkrp(h, d, factors, R, out, -1, st);
+    }
+    MK_TRY(ensure_layout(h, (d + h->N - 1) % h->N, st));
+    return launch_mttkrp(h, d, factors, R, out, h->cur, st);
 }
 
 }  // namespace mk
@@ -103,6 +116,10 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
     h->max_rank = max_rank;
     h->device = dev;
     h->timing = new (std::nothrow) Timing();
+    {
+        const char* env = getenv("MTTKRP_FUSE");          // MTTKRP_FUSE=0: always remap with the separate kernel
+        h->fuse = (env && env[0] == '0') ? 0 : 1;
+    }
     for (int d = 0; d < nmodes; ++d) {
         ModeMeta& mm = h->mode[d];
         choose_key_order(nmodes, dims, d, mm.order);
@@ -140,8 +157,7 @@ static mttkrp_status_t check_mode_args(mttkrp_handle_t h, int d, const float* co
 mttkrp_status_t mttkrp_mode(mttkrp_handle_t h, int d, const float* const* factors, int R, float* out, void* cuda_stream) {
     MK_TRY(check_mode_args(h, d, factors, R, out));
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    MK_TRY(ensure_layout(h, d, st));
-    return launch_mttkrp(h, d, factors, R, out, st);
+    return run_mode(h, d, factors, R, out, st);
 }
 
 mttkrp_status_t mttkrp_sweep(mttkrp_handle_t h, const float* const* factors, int R, float* const* outs, void* cuda_stream) {
@@ -173,8 +189,7 @@ mttkrp_status_t mttkrp_sweep_host(mttkrp_handle_t h, const float* const* factors
         dfac[m] = h->stage_fac[m];
     }
     for (int d = 0; d < h->N; ++d) {
-        MK_TRY(ensure_layout(h, d, st));
-        MK_TRY(launch_mttkrp(h, d, dfac, R, h->stage_out[d], st));
+        MK_TRY(run_mode(h, d, dfac, R, h->stage_out[d], st));
         MK_CUDA(cudaMemcpyAsync(outs[d], h->stage_out[d], (size_t)h->dims[d] * R * 4, cudaMemcpyDeviceToHost, st));
     }
     MK_CUDA(cudaStreamSynchronize(st));

@@ -89,6 +89,7 @@ struct mttkrp_handle_s {
     int64_t bytes_held;
     int64_t remaps_done;
     int device;
+    int fuse;                 // 1: remap inside the MTTKRP kernel when the call order is cyclic (default)
     mk::Timing* timing;       // owned; per-kernel event pairs while mttkrp_timing_begin is active
 };
 
@@ -115,7 +116,7 @@ mttkrp_status_t launch_export(const mttkrp_handle_s* h, int32_t* idx, float* val
 mttkrp_status_t launch_perm_step(const uint32_t* map, const uint32_t* in, uint32_t* out, int64_t nnz, cudaStream_t st);
 
 // ---- mttkrp_kernel.cu -----------------------------------------------------------------------
-mttkrp_status_t launch_mttkrp(const mttkrp_handle_s* h, int d, const float* const* factors, int R,
-                              float* out, cudaStream_t st);
+mttkrp_status_t launch_mttkrp(mttkrp_handle_s* h, int d, const float* const* factors, int R,
+                              float* out, int fuse_from, cudaStream_t st);
 
 }  // namespace mk

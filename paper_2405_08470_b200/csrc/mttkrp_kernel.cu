@@ -37,6 +37,15 @@ struct KernelArgs {
     const float* fac[N];     // fac[l] = factor of the mode at key level l (fac[0] unused)
     float* out;
     float* carry;            // [2*num_shards][R]
+    // Fused remap (Alg. 4 lines 17-19: elementwise computation and dynamic remapping in one kernel):
+    // rec is then T_in in the PREVIOUS layout, record j of this layout is T_in[prev[j]] with its
+    // index fields permuted (field l <- source field src[l]; dpos = inverse), and the kernel also
+    // writes it to rec_out[j] (T_out, this layout, padded).
+    const uint32_t* prev;    // [nnz_real] gather map
+    uint32_t* rec_out;
+    int64_t nnz_real;
+    int src[N];
+    uint32_t dpos_packed;    // 4 bits per source field: its level in this layout
 };
 
 // ---- small PTX helpers ------------------------------------------------------------------------
@@ -67,10 +76,11 @@ __device__ __forceinline__ Vec<V> vzero() {
     return r;
 }
 
-// One lane's V columns of factor row `row` (read-only path; 256-bit or 128-bit load).
+// One lane's V columns of a factor row (read-only path; 256-bit or 128-bit load).
+// `lanep` = factor base + this lane's column offset.
 template <int V>
-__device__ __forceinline__ Vec<V> ld_row(const float* __restrict__ A, uint32_t row, int R, int sub) {
-    const float* p = A + (size_t)row * R + sub * V;
+__device__ __forceinline__ Vec<V> ld_row(const float* __restrict__ lanep, uint32_t row, int R) {
+    const float* p = lanep + (size_t)row * R;
     Vec<V> r;
     if constexpr (V == 8) {
         asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
@@ -78,7 +88,7 @@ __device__ __forceinline__ Vec<V> ld_row(const float* __restrict__ A, uint32_t r
                        "=f"(r.p[3].x), "=f"(r.p[3].y)
                      : "l"(p));
     } else {
-        float4 v = __ldg(reinterpret_cast<const float4*>(p));
+        const float4 v = __ldg(reinterpret_cast<const float4*>(p));
         r.p[0] = make_float2(v.x, v.y);
         r.p[1] = make_float2(v.z, v.w);
     }
@@ -165,14 +175,17 @@ struct Rec {
     float val;
 };
 
-template <int N, int R>
+template <int N, int R, bool FUSED>
 __global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a) {
     using Ge = Geo<N, R>;
     constexpr int V = Ge::V, LPN = Ge::LPN, NPW = Ge::NPW, WARPS = Ge::WARPS, G = Ge::G, K = Ge::K;
     constexpr int STAGES = Ge::STAGES, RECW = Ge::RECW, SLOTW = Ge::SLOTW, NL = Ge::NL;
     constexpr int ROWW = NPW * SLOTW;                     // ring words between consecutive records of a group
     constexpr int STAGEW = K * ROWW;                      // ring words per stage
-    constexpr bool PIECE16 = (RECW % 4 == 0);             // 16-byte cp.async pieces, else 4-byte
+    // 16-byte cp.async pieces when the record is a multiple of 16 bytes, else 4-byte.  The fused
+    // variant permutes the index fields: for free at copy time with 4-byte pieces, and with selects
+    // after the LDS.128 for 3-mode records (kept as one 16-byte piece).
+    constexpr bool PIECE16 = FUSED ? (N == 3) : (RECW % 4 == 0);
     constexpr int PW = PIECE16 ? 4 : 1;                   // piece words
     constexpr int PPR = RECW / PW;                        // pieces per record
     constexpr int NPIECE = (K * PPR + LPN - 1) / LPN;     // pieces per lane per round
@@ -196,13 +209,31 @@ __global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a)
     const int64_t s_end = s_begin + a.shard_nnz;
     const int C = a.shard_nnz / G;                        // records per group; a multiple of K
     const int nrounds = C / K;
-    const uint32_t* const grec = a.rec + (size_t)(s_begin + (int64_t)(warp * NPW + g) * C) * RECW;
+    const int64_t cb = s_begin + (int64_t)(warp * NPW + g) * C;         // this group's first position
+    const uint32_t* const grec = a.rec + (size_t)cb * RECW;
+    const int n_real = FUSED ? (int)max((int64_t)0, min((int64_t)C, a.nnz_real - cb)) : C;   // rest is padding
 
     uint32_t* const ring = &s_warp[warp][0];
     const uint32_t* const ring_g = ring + g * SLOTW;      // this group's column of the ring
     const uint32_t ring_gs = (uint32_t)__cvta_generic_to_shared(ring_g);
 
-    auto issue_round = [&](int r) {
+    const int k0w = (FUSED && PIECE16) ? a.src[0] : 0;    // ring word holding k_0 (3-mode fused slots keep source order)
+
+    // fused: source positions of this lane's pieces, fetched two rounds before they are needed
+    uint32_t pvA[NPIECE], pvB[NPIECE];
+    auto load_prev = [&](int r, uint32_t* pv) {
+        if constexpr (FUSED) {
+#pragma unroll
+            for (int i = 0; i < NPIECE; ++i) {
+                const int p = sub + i * LPN;
+                const int jj = p / PPR;
+                int64_t j = cb + (int64_t)r * K + jj;
+                if (j > a.nnz_real - 1) j = a.nnz_real - 1;          // padding copies the last nonzero
+                pv[i] = (p < K * PPR && r < nrounds) ? __ldg(a.prev + j) : 0u;
+            }
+        }
+    };
+    auto issue_round = [&](int r, const uint32_t* pv) {
         if (r < nrounds) {
             const uint32_t* src = grec + (size_t)r * (K * RECW);
             const uint32_t dst = ring_gs + 4u * (uint32_t)((r & (STAGES - 1)) * STAGEW);
@@ -211,8 +242,14 @@ __global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a)
                 const int p = sub + i * LPN;
                 if (p < K * PPR) {
                     const int jj = p / PPR, q = p % PPR;
-                    if constexpr (PIECE16) cp_async16(dst + 4u * (uint32_t)(jj * ROWW + q * PW), src + jj * RECW + q * PW, true);
-                    else cp_async4(dst + 4u * (uint32_t)(jj * ROWW + q * PW), src + jj * RECW + q * PW, true);
+                    if constexpr (FUSED) {
+                        const uint32_t* s2 = a.rec + (size_t)pv[i] * RECW + q * PW;
+                        if constexpr (PIECE16) cp_async16(dst + 4u * (uint32_t)(jj * ROWW), s2, true);
+                        else cp_async4(dst + 4u * (uint32_t)(jj * ROWW + (q < N ? (int)((a.dpos_packed >> (4 * q)) & 15u) : N)), s2, true);
+                    } else {
+                        if constexpr (PIECE16) cp_async16(dst + 4u * (uint32_t)(jj * ROWW + q * PW), src + jj * RECW + q * PW, true);
+                        else cp_async4(dst + 4u * (uint32_t)(jj * ROWW + q * PW), src + jj * RECW + q * PW, true);
+                    }
                 }
             }
         }
@@ -227,11 +264,44 @@ __global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a)
             const uint4 v = p[i];
             w[4 * i] = v.x; w[4 * i + 1] = v.y; w[4 * i + 2] = v.z; w[4 * i + 3] = v.w;
         }
+        if constexpr (FUSED && N == 3) {                  // permute the index fields (uniform selects)
 #pragma unroll
-        for (int i = 0; i < N; ++i) r.k[i] = w[i];
+            for (int i = 0; i < 3; ++i) r.k[i] = a.src[i] == 0 ? w[0] : (a.src[i] == 1 ? w[1] : w[2]);
+        } else {
+#pragma unroll
+            for (int i = 0; i < N; ++i) r.k[i] = w[i];
+        }
         r.val = __uint_as_float(w[N]);
         return r;
     };
+    // fused: record j of this layout goes to T_out (one lane of the group, vector stores)
+    auto write_out = [&](int j, const Rec<N>& rc, float v) {
+        if constexpr (FUSED) {
+            if (sub == 0) {
+                uint32_t* o = a.rec_out + (size_t)(cb + j) * RECW;
+                uint32_t w[RECW];
+#pragma unroll
+                for (int i = 0; i < N; ++i) w[i] = rc.k[i];
+                w[N] = __float_as_uint(v);
+                if constexpr (RECW % 4 == 0) {
+#pragma unroll
+                    for (int i = 0; i < RECW / 4; ++i)
+                        __stcs(reinterpret_cast<uint4*>(o) + i, make_uint4(w[4 * i], w[4 * i + 1], w[4 * i + 2], w[4 * i + 3]));
+                } else if constexpr (RECW % 2 == 0) {
+#pragma unroll
+                    for (int i = 0; i < RECW / 2; ++i) __stcs(reinterpret_cast<uint2*>(o) + i, make_uint2(w[2 * i], w[2 * i + 1]));
+                } else {
+#pragma unroll
+                    for (int i = 0; i < RECW; ++i) __stcs(o + i, w[i]);
+                }
+            }
+        }
+    };
+
+    const float* facp[N];                                 // factor bases + this lane's column offset
+#pragma unroll
+    for (int l = 1; l < N; ++l) facp[l] = a.fac[l] + sub * V;
+    facp[0] = nullptr;
 
     Vec<V> t[NL];                                         // t[0] = output row accumulator
 #pragma unroll
@@ -253,11 +323,13 @@ __global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a)
             diff = diff || (nxt.k[l] != cur.k[l]);
             e |= diff ? (1u << l) : 0u;
         }
-        al[slot] = ld_row<V>(a.fac[N - 1], cur.k[N - 1], R, sub);
+        const float v = (!FUSED || j < n_real) ? cur.val : 0.f;      // padding records carry value 0
+        write_out(j, cur, v);
+        al[slot] = ld_row<V>(facp[N - 1], cur.k[N - 1], R);
 #pragma unroll
         for (int l = 1; l < NL; ++l)
-            if (e & (1u << l)) rb[l][slot] = ld_row<V>(a.fac[l], cur.k[l], R, sub);
-        val[slot] = cur.val;
+            if (e & (1u << l)) rb[l][slot] = ld_row<V>(facp[l], cur.k[l], R);
+        val[slot] = v;
         ef[slot] = e;
         cur = nxt;
     };
@@ -273,7 +345,7 @@ __global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a)
             }
         }
         if ((e & 1u) && j + 1 < C) {                      // an output row ends inside the chunk
-            const uint32_t row = jslot[0];
+            const uint32_t row = jslot[k0w];
             float* dst = (seg == 0) ? &s_first[warp][g][sub * V] : a.out + (size_t)row * R + sub * V;
             vstore<V>(dst, t[0]);
             if (seg == 0 && sub == 0) s_erow[warp][2 * g] = (int)row;
@@ -283,14 +355,24 @@ __global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a)
     };
 
 #pragma unroll
-    for (int r = 0; r < STAGES - 1; ++r) issue_round(r);
+    for (int r = 0; r < STAGES - 1; ++r) {
+        load_prev(r, pvA);
+        issue_round(r, pvA);
+    }
+    load_prev(STAGES - 1, pvA);
+    load_prev(STAGES, pvB);
     cp_async_wait<STAGES - 2>();                          // round 0 has landed
     __syncwarp();
     cur = read_rec(ring_g);
     lookahead(0, ring_g + 1 * ROWW, 0);
     lookahead(1, ring_g + 2 * ROWW, 1);
     for (int r = 0; r < nrounds; ++r) {
-        issue_round(r + STAGES - 1);
+        issue_round(r + STAGES - 1, pvA);
+        if constexpr (FUSED) {
+#pragma unroll
+            for (int i = 0; i < NPIECE; ++i) pvA[i] = pvB[i];
+            load_prev(r + STAGES + 1, pvB);
+        }
         cp_async_wait<STAGES - 2>();                      // rounds <= r+1 have landed
         __syncwarp();
         const uint32_t* cs = ring_g + (r & (STAGES - 1)) * STAGEW;          // this round's stage
@@ -308,7 +390,7 @@ __global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a)
         __syncwarp();                                     // everyone is done with round r's stage
     }
     cp_async_wait<0>();
-    const uint32_t last_row = ring_g[((C - 1) & (STAGES * K - 1)) * ROWW];
+    const uint32_t last_row = ring_g[((C - 1) & (STAGES * K - 1)) * ROWW + k0w];
     __syncwarp();
     // chunk epilogue: the still-open row goes to the first (seg == 0) or last partial-row entry
     float* const s_last = reinterpret_cast<float*>(ring);               // [NPW][R], aliases the ring
@@ -365,10 +447,20 @@ __global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a)
 
     // level 2: merge the warps' partial rows; rows shared with a neighbouring shard go to the carry buffer
     if (warp == 0) {
-        const uint32_t first_row = __ldg(a.rec + (size_t)s_begin * RECW);
-        const uint32_t end_row = __ldg(a.rec + (size_t)(s_end - 1) * RECW);
-        const bool head_shared = s_begin > 0 && __ldg(a.rec + (size_t)(s_begin - 1) * RECW) == first_row;
-        const bool tail_shared = s_end < a.nnz && __ldg(a.rec + (size_t)s_end * RECW) == end_row;
+        // output index of the record at position pos of THIS layout (fused: through the gather map,
+        // because the neighbouring shards may not have written T_out yet)
+        auto key0_at = [&](int64_t pos) {
+            if constexpr (FUSED) {
+                if (pos > a.nnz_real - 1) pos = a.nnz_real - 1;
+                return __ldg(a.rec + (size_t)__ldg(a.prev + pos) * RECW + a.src[0]);
+            } else {
+                return __ldg(a.rec + (size_t)pos * RECW);
+            }
+        };
+        const uint32_t first_row = key0_at(s_begin);
+        const uint32_t end_row = key0_at(s_end - 1);
+        const bool head_shared = s_begin > 0 && key0_at(s_begin - 1) == first_row;
+        const bool tail_shared = s_end < a.nnz && key0_at(s_end) == end_row;
         constexpr int CPL = (R + 31) / 32;
         merge_runs<R>(s_wrow, &s_wvec[0][0], 2 * WARPS, lane, [&](int row, const float* acc, bool, bool) {
             float* dst;
@@ -421,8 +513,21 @@ __global__ void __launch_bounds__(256) k_zero_rows(const uint32_t* __restrict__ 
         *(reinterpret_cast<float4*>(out + (size_t)rows[i] * R) + sub) = make_float4(0.f, 0.f, 0.f, 0.f);
 }
 
+template <int N, int R, bool FUSED>
+static mttkrp_status_t launch_main(const KernelArgs<N>& a, int64_t num_shards, Timing* timing, cudaStream_t st) {
+    constexpr int smem = Geo<N, R>::SMEM_BYTES;
+    static bool attr_set = false;
+    if (!attr_set) {
+        MK_CUDA(cudaFuncSetAttribute(k_mttkrp<N, R, FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        attr_set = true;
+    }
+    TimedLaunch tl(timing, kClsMttkrp, st);
+    k_mttkrp<N, R, FUSED><<<(unsigned)num_shards, kBlockThreads, smem, st>>>(a);
+    return MTTKRP_OK;
+}
+
 template <int N, int R>
-static mttkrp_status_t launch_nr(const mttkrp_handle_s* h, int d, const float* const* factors, float* out,
+static mttkrp_status_t launch_nr(mttkrp_handle_s* h, int d, const float* const* factors, float* out, int fuse_from,
                                  cudaStream_t st) {
     const ModeMeta& mm = h->mode[d];
     if (mm.n_empty > 0) {
@@ -441,48 +546,64 @@ static mttkrp_status_t launch_nr(const mttkrp_handle_s* h, int d, const float* c
         for (int l = 1; l < N; ++l) a.fac[l] = factors[mm.order[l]];
         a.out = out;
         a.carry = h->carry;
-        {
-            constexpr int smem = Geo<N, R>::SMEM_BYTES;
-            static bool attr_set = false;
-            if (!attr_set) {
-                MK_CUDA(cudaFuncSetAttribute(k_mttkrp<N, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-                attr_set = true;
-            }
-            TimedLaunch tl(h->timing, kClsMttkrp, st);
-            k_mttkrp<N, R><<<(unsigned)h->num_shards, kBlockThreads, smem, st>>>(a);
+        a.prev = nullptr;
+        a.rec_out = nullptr;
+        a.nnz_real = h->nnz;
+        a.dpos_packed = 0;
+        for (int l = 0; l < N; ++l) { a.src[l] = l; a.dpos_packed |= (uint32_t)l << (4 * l); }
+        if (fuse_from >= 0) {
+            // remap fuse_from -> d inside the MTTKRP kernel; T_out becomes the resident copy
+            a.prev = h->mode[fuse_from].next;
+            a.rec_out = h->rec_alt;
+            for (int l = 0; l < N; ++l) a.src[l] = h->mode[fuse_from].pos[mm.order[l]];
+            a.dpos_packed = 0;
+            for (int l = 0; l < N; ++l) a.dpos_packed |= (uint32_t)l << (4 * a.src[l]);
+            MK_TRY((launch_main<N, R, true>(a, h->num_shards, h->timing, st)));
+            uint32_t* t = h->rec_cur;      // swap(T_in, T_out), Alg. 5 line 12
+            h->rec_cur = h->rec_alt;
+            h->rec_alt = t;
+            h->cur = d;
+            h->remaps_done++;
+        } else {
+            MK_TRY((launch_main<N, R, false>(a, h->num_shards, h->timing, st)));
         }
         if (mm.n_chains > 0) {
             TimedLaunch tl(h->timing, kClsFixup, st);
             k_fixup<R><<<(unsigned)mm.n_chains, 128, 0, st>>>(mm.chains, h->carry, out);
         }
+    } else if (fuse_from >= 0) {
+        h->cur = d;
+        h->remaps_done++;
     }
     MK_CUDA(cudaGetLastError());
     return MTTKRP_OK;
 }
 
 template <int N>
-static mttkrp_status_t launch_n(const mttkrp_handle_s* h, int d, const float* const* factors, int R, float* out,
+static mttkrp_status_t launch_n(mttkrp_handle_s* h, int d, const float* const* factors, int R, float* out, int fuse_from,
                                 cudaStream_t st) {
     switch (R) {
-        case 8: return launch_nr<N, 8>(h, d, factors, out, st);
-        case 16: return launch_nr<N, 16>(h, d, factors, out, st);
-        case 32: return launch_nr<N, 32>(h, d, factors, out, st);
-        case 64: return launch_nr<N, 64>(h, d, factors, out, st);
+        case 8: return launch_nr<N, 8>(h, d, factors, out, fuse_from, st);
+        case 16: return launch_nr<N, 16>(h, d, factors, out, fuse_from, st);
+        case 32: return launch_nr<N, 32>(h, d, factors, out, fuse_from, st);
+        case 64: return launch_nr<N, 64>(h, d, factors, out, fuse_from, st);
     }
     set_error("unsupported rank %d (8, 16, 32, 64)", R);
     return MTTKRP_EUNSUPPORTED;
 }
 
-mttkrp_status_t launch_mttkrp(const mttkrp_handle_s* h, int d, const float* const* factors, int R, float* out,
+// fuse_from < 0: the resident copy is already in layout d.  fuse_from >= 0: it is in layout
+// fuse_from with (fuse_from + 1) % N == d, and the remap is done inside the MTTKRP kernel.
+mttkrp_status_t launch_mttkrp(mttkrp_handle_s* h, int d, const float* const* factors, int R, float* out, int fuse_from,
                               cudaStream_t st) {
     switch (h->N) {
-        case 2: return launch_n<2>(h, d, factors, R, out, st);
-        case 3: return launch_n<3>(h, d, factors, R, out, st);
-        case 4: return launch_n<4>(h, d, factors, R, out, st);
-        case 5: return launch_n<5>(h, d, factors, R, out, st);
-        case 6: return launch_n<6>(h, d, factors, R, out, st);
-        case 7: return launch_n<7>(h, d, factors, R, out, st);
-        case 8: return launch_n<8>(h, d, factors, R, out, st);
+        case 2: return launch_n<2>(h, d, factors, R, out, fuse_from, st);
+        case 3: return launch_n<3>(h, d, factors, R, out, fuse_from, st);
+        case 4: return launch_n<4>(h, d, factors, R, out, fuse_from, st);
+        case 5: return launch_n<5>(h, d, factors, R, out, fuse_from, st);
+        case 6: return launch_n<6>(h, d, factors, R, out, fuse_from, st);
+        case 7: return launch_n<7>(h, d, factors, R, out, fuse_from, st);
+        case 8: return launch_n<8>(h, d, factors, R, out, fuse_from, st);
     }
     set_error("unsupported nmodes %d", h->N);
     return MTTKRP_EUNSUPPORTED;
