@@ -89,7 +89,7 @@ struct mttkrp_handle_s {
     int64_t bytes_held;
     int64_t remaps_done;
     int device;
-    int fuse;                 // 1: remap inside the MTTKRP kernel when the call order is cyclic (default)
+    int fuse;                 // 1: last remap step inside the MTTKRP kernel (opt-in, MTTKRP_FUSE=1)
     mk::Timing* timing;       // owned; per-kernel event pairs while mttkrp_timing_begin is active
 };
 
