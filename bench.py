@@ -177,25 +177,20 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 def run_ours(args):
     import torch
-    import torch.distributed as dist
     import workloads as W
     import paper_2405_08470_b200 as P
+    from paper_2405_08470_b200 import replicas
 
     P.load_library()                                   # fail loudly if the CUDA library is missing
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    _, _, local = replicas.env_ranks()
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+    rank, world, local = replicas.init("nccl", dev)
 
     def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+        replicas.barrier(dev)
 
     spec = W.CONFIGS[args.config]
     if args.nnz:
@@ -248,10 +243,7 @@ def run_ours(args):
     w1 = time.time()
     ms_total = e0.elapsed_time(e1)
     clocks = sampler.stop(w0, w1)
-    if world > 1:
-        tt = torch.tensor([ms_total], device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms_total = float(tt.item())
+    ms_total = replicas.max_over_ranks(ms_total, dev)
     ms_step = ms_total / args.steps
     value = world * flops_per_sweep / (ms_step * 1e-3) / 1e9
 
@@ -302,10 +294,7 @@ def run_ours(args):
         e1.record()
         barrier()
         ms_e2e = e0.elapsed_time(e1)
-        if world > 1:
-            tt = torch.tensor([ms_e2e], device=dev)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            ms_e2e = float(tt.item())
+        ms_e2e = replicas.max_over_ranks(ms_e2e, dev)
         io = sum(d * R * 4 for d in spec.dims)
         e2e = {"value": world * flops_per_sweep / (ms_e2e / args.steps * 1e-3) / 1e9, "unit": UNIT,
                "h2d_bytes_per_step": io, "d2h_bytes_per_step": io, "ms_per_step": ms_e2e / args.steps,
@@ -333,8 +322,7 @@ def run_ours(args):
                                  "(PAPER.md:414); no absolute numbers published"}
         print(json.dumps(line), flush=True)
     h.destroy()
-    if world > 1:
-        dist.destroy_process_group()
+    replicas.finalize()
 
 
 def main():

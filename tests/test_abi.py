@@ -1,0 +1,103 @@
+"""CPU-only checks of the boundary: the C-ABI library loads, exports every symbol the header
+declares, and rejects bad arguments before touching CUDA (no compute calls without a GPU)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "mttkrp.h")
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2405_08470_b200 import build
+    build.build()                                  # nvcc cross-compiles for sm_100a without a GPU
+    import paper_2405_08470_b200 as P
+    return P.load_library()
+
+
+def _declared_symbols():
+    text = open(HEADER).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(mttkrp_[a-z_]+)\s*\(", text)))
+
+
+def test_header_symbols_are_all_exported(lib):
+    import paper_2405_08470_b200 as P
+    names = _declared_symbols()
+    assert len(names) >= 12 and "mttkrp_create" in names and "mttkrp_mode" in names and "mttkrp_destroy" in names
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in include/mttkrp.h but not exported"
+    assert sorted(P.EXPORTS) == names                      # the binding covers the same set
+    assert b"sm_100a" in lib.mttkrp_version()
+
+
+def test_workspace_bytes_is_host_arithmetic(lib):
+    import paper_2405_08470_b200 as P
+    a = P.mttkrp_workspace_bytes([1000, 800, 600], 100_000)
+    b = P.mttkrp_workspace_bytes([1000, 800, 600], 200_000)
+    c = P.mttkrp_workspace_bytes([1000, 800, 600], 100_000, max_rank=32)
+    assert 0 < a < b and c > a
+    # two padded tensor copies + N maps + perm0 at least
+    assert a >= 100_000 * (2 * 16 + 3 * 4 + 4)
+    assert c - a >= 2 * (1000 + 800 + 600) * 32 * 4        # factor + output staging
+    assert P.mttkrp_workspace_bytes([5, 4, 3], 0) > 0      # nnz == 0 is legal
+    big = P.mttkrp_workspace_bytes([4_800_000, 1_800_000, 1_800_000], 200_000_000)
+    assert 9e9 < big < 20e9                                # config 3 fits a 180 GB GPU many times over
+
+
+@pytest.mark.parametrize("dims,nnz,rank,status", [
+    ([10], 5, 0, 3),                 # nmodes < 2 -> EUNSUPPORTED
+    ([2] * 9, 5, 0, 3),              # nmodes > 8
+    ([10, 0, 3], 5, 0, 1),           # non-positive dim -> EINVAL
+    ([10, 4, 3], -1, 0, 1),          # nnz < 0
+    ([10, 4, 3], 2**31, 0, 3),       # nnz >= 2^31
+    ([10, 4, 3], 5, 12, 3),          # bad max_rank
+])
+def test_bad_shapes_are_rejected(lib, dims, nnz, rank, status):
+    import paper_2405_08470_b200 as P
+    with pytest.raises(P.MttkrpError) as e:
+        P.mttkrp_workspace_bytes(dims, nnz, rank)
+    assert e.value.status == status
+    assert str(e.value)
+
+
+def test_null_arguments_return_status_not_crash(lib):
+    out = ctypes.c_void_p(None)
+    dims = (ctypes.c_int64 * 3)(5, 4, 3)
+    # NULL workspace
+    st = lib.mttkrp_create(ctypes.byref(out), 3, dims, 10, ctypes.c_void_p(256), ctypes.c_void_p(256), 0, None, 0, None)
+    assert st == 4 and out.value is None and b"workspace" in lib.mttkrp_last_error()
+    # NULL idx with nnz > 0
+    st = lib.mttkrp_create(ctypes.byref(out), 3, dims, 10, None, None, 0, ctypes.c_void_p(256), 1 << 20, None)
+    assert st == 1
+    # misaligned workspace
+    st = lib.mttkrp_create(ctypes.byref(out), 3, dims, 10, ctypes.c_void_p(256), ctypes.c_void_p(256), 0, ctypes.c_void_p(8), 1 << 30, None)
+    assert st == 4
+    # workspace too small
+    st = lib.mttkrp_create(ctypes.byref(out), 3, dims, 10, ctypes.c_void_p(256), ctypes.c_void_p(256), 0, ctypes.c_void_p(256), 16, None)
+    assert st == 4 and b"required" in lib.mttkrp_last_error()
+    # NULL handle everywhere
+    assert lib.mttkrp_destroy(None) == 1
+    assert lib.mttkrp_mode(None, 0, None, 32, None, None) == 1
+    assert lib.mttkrp_sweep(None, None, 32, None, None) == 1
+    assert lib.mttkrp_remap_to(None, 0, None) == 1
+    assert lib.mttkrp_get_info(None, None) == 1
+    assert lib.mttkrp_timing_begin(None) == 1
+
+
+def test_product_path_has_no_cpu_fallback():
+    import torch
+    import paper_2405_08470_b200 as P
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(RuntimeError):
+        P.Mttkrp([5, 4, 3], torch.zeros((3, 1), dtype=torch.int32), torch.zeros(1))
+    # and nothing under the package imports the oracle
+    pkg = os.path.join(ROOT, "paper_2405_08470_b200")
+    for dp, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                assert "oracle" not in open(os.path.join(dp, f)).read().lower(), f
