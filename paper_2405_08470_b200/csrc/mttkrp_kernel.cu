@@ -2,21 +2,23 @@
 // Alg. 4 thread-block mapping, as function only; the mapping here is this
 // library's own, made for sm_100a).
 //
-// Layout: records sorted by the key tuple (k_0 = i_d, k_1, ..., k_{N-1}); record = N int32 keys in
-// that order + fp32 value.  A thread block owns one shard = shard_nnz consecutive records
-// (equal-nnz shards).  Inside the block a GROUP of R/V lanes (V = 8 rank columns per lane, one
-// 256-bit LDG per factor row per lane) walks a contiguous chunk of the shard one nonzero at a time:
+// Layout: records sorted by the key tuple (k_0 = i_d, k_1, ..., k_{N-1}); record = N uint32 keys in
+// that order + fp32 value.  In shared memory bit 31 of the key words carries the run-end flags, which a
+// per-stage fix-up pass derives from the sorted order once per record, so in the hot loop a record is
+// self-contained: no look-ahead compare in the hot loop.
+// A thread block owns one shard = shard_nnz consecutive records (equal-nnz shards).  Inside the
+// block a GROUP of R/V lanes (V = 8 rank columns per lane, one 256-bit LDG per factor row per lane)
+// walks a contiguous chunk of the shard one nonzero at a time:
 //   l(r) = val * prod_w A_w[i_w, r]         (Alg. 2 lines 8-13)
 //   Y_d[i_d, r] += l(r)                     (Alg. 2 lines 14-15)
 // Because the chunk is sorted, the products are nested sums (a CSF-style factoring of the same
 // expression):  Y[k_0] = sum_{k_1} A[k_1] * ( sum_{k_2} A[k_2] * ( ... sum_{k_{N-1}} val * A[k_{N-1}] ) ),
 // so the row of level l is gathered once per run of equal (k_0..k_l), at the END of the run.
 //
-// Pipeline per warp: records are staged into a shared-memory ring with cp.async (4 stages of 4
-// records per group, interleaved by group so one LDS.128 serves all groups without bank conflicts);
-// two steps ahead of the arithmetic the group reads record j and j+1 from the ring, derives the
-// end-of-run flags, and issues the factor-row gathers for step j into rotating registers.
-// The arithmetic is packed fp32x2 FMA (FFMA2).
+// Pipeline per warp: records are staged into a shared-memory ring with cp.async (4-6 stages of K
+// records per group, interleaved by group so one LDS.128 serves all groups without bank conflicts).
+// D steps ahead of the arithmetic the group reads its record from the ring and issues the
+// factor-row gathers for that step into rotating registers.  The arithmetic is packed fp32x2 FMA.
 //
 // Rows that begin and end inside a chunk are stored with plain stores by their only owner
 // (Observation 2: no global atomics).  The first/last partial rows of each chunk
@@ -37,15 +39,6 @@ struct KernelArgs {
     const float* fac[N];     // fac[l] = factor of the mode at key level l (fac[0] unused)
     float* out;
     float* carry;            // [2*num_shards][R]
-    // Fused remap (Alg. 4 lines 17-19: elementwise computation and dynamic remapping in one kernel):
-    // rec is then T_in in the PREVIOUS layout, record j of this layout is T_in[prev[j]] with its
-    // index fields permuted (field l <- source field src[l]; dpos = inverse), and the kernel also
-    // writes it to rec_out[j] (T_out, this layout, padded).
-    const uint32_t* prev;    // [nnz_real] gather map
-    uint32_t* rec_out;
-    int64_t nnz_real;
-    int src[N];
-    uint32_t dpos_packed;    // 4 bits per source field: its level in this layout
 };
 
 // ---- small PTX helpers ------------------------------------------------------------------------
@@ -77,10 +70,12 @@ __device__ __forceinline__ Vec<V> vzero() {
 }
 
 // One lane's V columns of a factor row (read-only path; 256-bit or 128-bit load).
-// `lanep` = factor base + this lane's column offset.
-template <int V>
-__device__ __forceinline__ Vec<V> ld_row(const float* __restrict__ lanep, uint32_t row, int R) {
-    const float* p = lanep + (size_t)row * R;
+// `lanep` = factor base + this lane's column offset; `word` = row index, bit 31 (run-end flag) ignored:
+// address = lanep + (word << 1) * (R * 2) bytes, one shift and one 32x32->64 multiply-add.
+template <int V, int R>
+__device__ __forceinline__ Vec<V> ld_row(const float* __restrict__ lanep, uint32_t word) {
+    const float* p;
+    asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(p) : "r"(word << 1), "n"(R * 2), "l"(lanep));
     Vec<V> r;
     if constexpr (V == 8) {
         asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
@@ -113,28 +108,34 @@ __device__ __forceinline__ void vstore(float* dst, const Vec<V>& v) {
         *reinterpret_cast<float4*>(dst + 4 * i) = make_float4(v.p[2 * i].x, v.p[2 * i].y, v.p[2 * i + 1].x, v.p[2 * i + 1].y);
 }
 
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, bool pred) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(pred ? 16 : 0) : "memory");
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
-__device__ __forceinline__ void cp_async4(uint32_t dst, const void* src, bool pred) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(dst), "l"(src), "r"(pred ? 4 : 0) : "memory");
+__device__ __forceinline__ void cp_async8(uint32_t dst, const void* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async4(uint32_t dst, const void* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int NPEND>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(NPEND) : "memory"); }
 
 // ---- compile-time geometry ---------------------------------------------------------------------
-template <int N, int R>
+template <int N, int R, bool FUSED>
 struct Geo {
     static constexpr int V = (R >= 16) ? 8 : 4;          // rank columns per lane
     static constexpr int LPN = R / V;                    // lanes per nonzero (group size)
     static constexpr int NPW = 32 / LPN;                 // groups per warp
     static constexpr int WARPS = kBlockThreads / 32;
     static constexpr int G = WARPS * NPW;                // groups per block
-    static constexpr int K = 4;                          // records per group per ring stage
-    static constexpr int STAGES = 4;
     static constexpr int RECW = N + 1;                   // record words
     static constexpr int SLOTW = (RECW + 3) / 4 * 4;     // ring slot words (16-byte multiple)
+    static constexpr int K = (NPW * SLOTW <= 32 || NPW < 8) ? 8 : 4;  // records per group per ring stage
+    // ring stages: round r computing, r+1 fixed up, r+2 landed, the rest in flight (the fused variant
+    // gathers records from random DRAM positions and keeps more rounds in flight)
+    static constexpr int STAGES = (FUSED && K * NPW * SLOTW * 4 <= 1024) ? 6 : 4;
+    static constexpr int D = 2;                          // gather look-ahead, in steps (K % D == 0)
     static constexpr int RING_WORDS = STAGES * K * NPW * SLOTW;        // per warp
     static constexpr int ENT_WORDS = 2 * NPW * R;                       // per warp: first/last partial rows
     static constexpr int WARP_WORDS = RING_WORDS > ENT_WORDS ? RING_WORDS : ENT_WORDS;
@@ -169,27 +170,37 @@ __device__ __forceinline__ void merge_runs(const int* rows, const float* vecs, i
     if (cur_row >= 0) emit(cur_row, acc, run == 0, true);
 }
 
+constexpr uint32_t kFlag = 0x80000000u;   // run-end flag bit inside a key word (shared memory only)
+
+// FUSED = false: `rec` is the tensor copy already in this mode's layout (after a separate remap pass).
+// FUSED = true : dynamic remapping inside the kernel (Alg. 4 lines 17-19: elementwise
+//   computation and dynamic remapping in one kernel).  `rec` is T_in in the PREVIOUS layout; record j of
+//   this layout is T_in[prev[j]] with its index fields permuted (field l <- source field src[l]); the
+//   kernel gathers it straight into the shared-memory ring with cp.async and also writes it to
+//   rec_out[j] (T_out, this layout), which is the next mode's T_in.
 template <int N>
-struct Rec {
-    uint32_t k[N];
-    float val;
+struct FuseArgs {
+    const uint32_t* prev;    // [nnz_real] gather map
+    uint32_t* rec_out;       // padded like rec
+    int64_t nnz_real;
+    int src[N];
+    uint32_t dpos_packed;    // 4 bits per source field: its level in this layout
 };
 
 template <int N, int R, bool FUSED>
-__global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a) {
-    using Ge = Geo<N, R>;
-    constexpr int V = Ge::V, LPN = Ge::LPN, NPW = Ge::NPW, WARPS = Ge::WARPS, G = Ge::G, K = Ge::K;
+__global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a, const FuseArgs<N> fa) {
+    using Ge = Geo<N, R, FUSED>;
+    constexpr int V = Ge::V, LPN = Ge::LPN, NPW = Ge::NPW, WARPS = Ge::WARPS, G = Ge::G, K = Ge::K, D = Ge::D;
     constexpr int STAGES = Ge::STAGES, RECW = Ge::RECW, SLOTW = Ge::SLOTW, NL = Ge::NL;
     constexpr int ROWW = NPW * SLOTW;                     // ring words between consecutive records of a group
     constexpr int STAGEW = K * ROWW;                      // ring words per stage
-    // 16-byte cp.async pieces when the record is a multiple of 16 bytes, else 4-byte.  The fused
-    // variant permutes the index fields: for free at copy time with 4-byte pieces, and with selects
-    // after the LDS.128 for 3-mode records (kept as one 16-byte piece).
-    constexpr bool PIECE16 = FUSED ? (N == 3) : (RECW % 4 == 0);
-    constexpr int PW = PIECE16 ? 4 : 1;                   // piece words
+    constexpr int RPL = K * NPW / 32;                     // records per lane per stage in the fix-up pass
+    // cp.async piece: the widest power of two dividing the record; the fused variant permutes the
+    // index fields for free at copy time with 4-byte pieces, and with selects for 16-byte records.
+    constexpr int PW = FUSED ? (N == 3 ? 4 : 1) : (RECW % 4 == 0 ? 4 : (RECW % 2 == 0 ? 2 : 1));
     constexpr int PPR = RECW / PW;                        // pieces per record
     constexpr int NPIECE = (K * PPR + LPN - 1) / LPN;     // pieces per lane per round
-    static_assert(K == 4 && STAGES == 4, "the step schedule below is written for 4 stages of 4 records");
+    static_assert(K % D == 0 && RPL >= 1 && K * NPW % 32 == 0, "geometry");
 
     extern __shared__ uint4 smem_raw[];
     // carve-up (Geo::SMEM_BYTES): record rings (later the groups' last partial rows) | the groups'
@@ -209,34 +220,32 @@ __global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a)
     const int64_t s_end = s_begin + a.shard_nnz;
     const int C = a.shard_nnz / G;                        // records per group; a multiple of K
     const int nrounds = C / K;
-    const int64_t cb = s_begin + (int64_t)(warp * NPW + g) * C;         // this group's first position
-    const uint32_t* const grec = a.rec + (size_t)cb * RECW;
-    const int n_real = FUSED ? (int)max((int64_t)0, min((int64_t)C, a.nnz_real - cb)) : C;   // rest is padding
+    const int64_t wb = s_begin + (int64_t)(warp * NPW) * C;             // first position of this warp's groups
+    const int64_t cb = wb + (int64_t)g * C;                             // this group's first position
 
     uint32_t* const ring = &s_warp[warp][0];
-    const uint32_t* const ring_g = ring + g * SLOTW;      // this group's column of the ring
+    uint32_t* const ring_g = ring + g * SLOTW;            // this group's column of the ring
     const uint32_t ring_gs = (uint32_t)__cvta_generic_to_shared(ring_g);
 
-    const int k0w = (FUSED && PIECE16) ? a.src[0] : 0;    // ring word holding k_0 (3-mode fused slots keep source order)
-
-    // fused: source positions of this lane's pieces, fetched two rounds before they are needed
-    uint32_t pvA[NPIECE], pvB[NPIECE];
-    auto load_prev = [&](int r, uint32_t* pv) {
+    // ---- record staging -------------------------------------------------------------------------
+    // fused: source positions of this lane's pieces, fetched one round before they are needed
+    uint32_t pv[NPIECE];
+    auto load_prev = [&](int r) {
         if constexpr (FUSED) {
 #pragma unroll
             for (int i = 0; i < NPIECE; ++i) {
                 const int p = sub + i * LPN;
                 const int jj = p / PPR;
                 int64_t j = cb + (int64_t)r * K + jj;
-                if (j > a.nnz_real - 1) j = a.nnz_real - 1;          // padding copies the last nonzero
-                pv[i] = (p < K * PPR && r < nrounds) ? __ldg(a.prev + j) : 0u;
+                if (j > fa.nnz_real - 1) j = fa.nnz_real - 1;        // padding copies the last nonzero
+                pv[i] = (p < K * PPR && r < nrounds) ? __ldcs(fa.prev + j) : 0u;
             }
         }
     };
-    auto issue_round = [&](int r, const uint32_t* pv) {
+    auto issue_round = [&](int r) {
         if (r < nrounds) {
-            const uint32_t* src = grec + (size_t)r * (K * RECW);
-            const uint32_t dst = ring_gs + 4u * (uint32_t)((r & (STAGES - 1)) * STAGEW);
+            const uint32_t* src = a.rec + (size_t)(cb + (int64_t)r * K) * RECW;
+            const uint32_t dst = ring_gs + 4u * (uint32_t)((r % STAGES) * STAGEW);
 #pragma unroll
             for (int i = 0; i < NPIECE; ++i) {
                 const int p = sub + i * LPN;
@@ -244,57 +253,102 @@ __global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a)
                     const int jj = p / PPR, q = p % PPR;
                     if constexpr (FUSED) {
                         const uint32_t* s2 = a.rec + (size_t)pv[i] * RECW + q * PW;
-                        if constexpr (PIECE16) cp_async16(dst + 4u * (uint32_t)(jj * ROWW), s2, true);
-                        else cp_async4(dst + 4u * (uint32_t)(jj * ROWW + (q < N ? (int)((a.dpos_packed >> (4 * q)) & 15u) : N)), s2, true);
+                        if constexpr (PW == 4) cp_async16(dst + 4u * (uint32_t)(jj * ROWW), s2);
+                        else cp_async4(dst + 4u * (uint32_t)(jj * ROWW + (q < N ? (int)((fa.dpos_packed >> (4 * q)) & 15u) : N)), s2);
                     } else {
-                        if constexpr (PIECE16) cp_async16(dst + 4u * (uint32_t)(jj * ROWW + q * PW), src + jj * RECW + q * PW, true);
-                        else cp_async4(dst + 4u * (uint32_t)(jj * ROWW + q * PW), src + jj * RECW + q * PW, true);
+                        const uint32_t d2 = dst + 4u * (uint32_t)(jj * ROWW + q * PW);
+                        if constexpr (PW == 4) cp_async16(d2, src + jj * RECW + q * PW);
+                        else if constexpr (PW == 2) cp_async8(d2, src + jj * RECW + q * PW);
+                        else cp_async4(d2, src + jj * RECW + q * PW);
                     }
                 }
             }
         }
         cp_async_commit();
     };
-    auto read_rec = [&](const uint32_t* slot) {
-        Rec<N> r;
-        uint32_t w[SLOTW];
+    auto read_slot = [&](const uint32_t* slot, uint32_t* w) {
         const uint4* p = reinterpret_cast<const uint4*>(slot);
 #pragma unroll
         for (int i = 0; i < SLOTW / 4; ++i) {
             const uint4 v = p[i];
             w[4 * i] = v.x; w[4 * i + 1] = v.y; w[4 * i + 2] = v.z; w[4 * i + 3] = v.w;
         }
-        if constexpr (FUSED && N == 3) {                  // permute the index fields (uniform selects)
-#pragma unroll
-            for (int i = 0; i < 3; ++i) r.k[i] = a.src[i] == 0 ? w[0] : (a.src[i] == 1 ? w[1] : w[2]);
-        } else {
-#pragma unroll
-            for (int i = 0; i < N; ++i) r.k[i] = w[i];
-        }
-        r.val = __uint_as_float(w[N]);
-        return r;
     };
-    // fused: record j of this layout goes to T_out (one lane of the group, vector stores)
-    auto write_out = [&](int j, const Rec<N>& rc, float v) {
-        if constexpr (FUSED) {
-            if (sub == 0) {
-                uint32_t* o = a.rec_out + (size_t)(cb + j) * RECW;
-                uint32_t w[RECW];
+    // Fix-up pass over stage r (all of it has landed, and so has record 0 of stage r+1): every lane
+    // takes RPL records, puts the keys into this layout's order (fused), derives the run-end flags
+    // from the following record of the same group and stores them in bit 31 of the key words
+    // (flag e_l in word l for 1 <= l <= N-2, e_0 in word N-1), and (fused) writes the record to T_out.
+    // The chunk's last record closes every inner run and leaves the output row open (epilogue).
+    auto fix_round = [&](int r) {
+        if (r >= nrounds) return;
+        uint32_t* const st = ring + (r % STAGES) * STAGEW;
+        const uint32_t* const stn = ring + ((r + 1) % STAGES) * STAGEW;
 #pragma unroll
-                for (int i = 0; i < N; ++i) w[i] = rc.k[i];
-                w[N] = __float_as_uint(v);
+        for (int i = 0; i < RPL; ++i) {
+            const int q = lane + 32 * i;
+            const int jj = q / NPW, gg = q % NPW;
+            uint32_t* slot = st + jj * ROWW + gg * SLOTW;
+            const uint32_t* nslot = (jj + 1 < K) ? slot + ROWW : stn + gg * SLOTW;
+            uint32_t w[SLOTW], nx[SLOTW];
+            read_slot(slot, w);
+            read_slot(nslot, nx);                          // stale past the chunk end; masked by `last`
+            __syncwarp();                                  // every lane has read before any slot is rewritten
+            uint32_t k[N], nk[N];
+            if constexpr (FUSED && N == 3) {               // permute the index fields (uniform selects)
+#pragma unroll
+                for (int l = 0; l < 3; ++l) {
+                    k[l] = fa.src[l] == 0 ? w[0] : (fa.src[l] == 1 ? w[1] : w[2]);
+                    nk[l] = fa.src[l] == 0 ? nx[0] : (fa.src[l] == 1 ? nx[1] : nx[2]);
+                }
+            } else {
+#pragma unroll
+                for (int l = 0; l < N; ++l) { k[l] = w[l]; nk[l] = nx[l]; }
+            }
+            uint32_t val = w[N];
+            const bool last = (r == nrounds - 1) && (jj == K - 1);
+            const int64_t pos = wb + (int64_t)gg * C + (int64_t)r * K + jj;
+            if constexpr (FUSED) {
+                if (pos >= fa.nnz_real) val = 0u;          // padding records carry value 0
+                uint32_t* o = fa.rec_out + (size_t)pos * RECW;
                 if constexpr (RECW % 4 == 0) {
+                    uint32_t ww[RECW];
 #pragma unroll
-                    for (int i = 0; i < RECW / 4; ++i)
-                        __stcs(reinterpret_cast<uint4*>(o) + i, make_uint4(w[4 * i], w[4 * i + 1], w[4 * i + 2], w[4 * i + 3]));
+                    for (int l = 0; l < N; ++l) ww[l] = k[l];
+                    ww[N] = val;
+#pragma unroll
+                    for (int c4 = 0; c4 < RECW / 4; ++c4)
+                        __stcs(reinterpret_cast<uint4*>(o) + c4, make_uint4(ww[4 * c4], ww[4 * c4 + 1], ww[4 * c4 + 2], ww[4 * c4 + 3]));
                 } else if constexpr (RECW % 2 == 0) {
+                    uint32_t ww[RECW];
 #pragma unroll
-                    for (int i = 0; i < RECW / 2; ++i) __stcs(reinterpret_cast<uint2*>(o) + i, make_uint2(w[2 * i], w[2 * i + 1]));
+                    for (int l = 0; l < N; ++l) ww[l] = k[l];
+                    ww[N] = val;
+#pragma unroll
+                    for (int c2 = 0; c2 < RECW / 2; ++c2) __stcs(reinterpret_cast<uint2*>(o) + c2, make_uint2(ww[2 * c2], ww[2 * c2 + 1]));
                 } else {
 #pragma unroll
-                    for (int i = 0; i < RECW; ++i) __stcs(o + i, w[i]);
+                    for (int l = 0; l < N; ++l) __stcs(o + l, k[l]);
+                    __stcs(o + N, val);
                 }
             }
+            bool diff = false;
+            uint32_t o4[SLOTW];
+#pragma unroll
+            for (int l = 0; l < SLOTW; ++l) o4[l] = 0u;
+            o4[0] = k[0];
+            bool e0 = false;
+#pragma unroll
+            for (int l = 0; l < NL; ++l) {
+                diff = diff || (nk[l] != k[l]);
+                const bool e = last ? (l > 0) : diff;
+                if (l == 0) e0 = e;
+                else o4[l] = k[l] | (e ? kFlag : 0u);
+            }
+            o4[N - 1] = k[N - 1] | (e0 ? kFlag : 0u);
+            o4[N] = val;
+#pragma unroll
+            for (int c4 = 0; c4 < SLOTW / 4; ++c4)
+                reinterpret_cast<uint4*>(slot)[c4] = make_uint4(o4[4 * c4], o4[4 * c4 + 1], o4[4 * c4 + 2], o4[4 * c4 + 3]);
         }
     };
 
@@ -306,91 +360,86 @@ __global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a)
     Vec<V> t[NL];                                         // t[0] = output row accumulator
 #pragma unroll
     for (int l = 0; l < NL; ++l) t[l] = vzero<V>();
-    Vec<V> al[2];                                         // last-level rows for the two steps in flight
-    Vec<V> rb[NL][2];                                     // rb[l][slot]: row of level l, gathered at the end of its run
-    float val[2] = {0.f, 0.f};
-    unsigned ef[2] = {0u, 0u};                            // bit l: the run of level l ends at this step
-    Rec<N> cur;
+    Vec<V> al[D];                                         // last-level rows for the D steps in flight
+    Vec<V> rb[NL][D];                                     // rb[l][slot]: row of level l, gathered at the end of its run
+    float val[D];
+    uint32_t fl[D];                                       // bit l: the run of level l ends at this step
     int seg = 0;                                          // output-row segments finished in this chunk
 
-    // Prepare step j (record `cur`; `nslot` holds record j+1): end-of-run flags and the row gathers.
-    auto lookahead = [&](int j, const uint32_t* nslot, int slot) {
-        const Rec<N> nxt = read_rec(nslot);               // stale past the chunk end; masked by `last`
-        unsigned e = 0u;
-        bool diff = (j + 1 >= C);
+    // Issue the gathers of one step whose (fixed-up) record sits at `slot`.
+    auto prefetch = [&](const uint32_t* slot, int s) {
+        uint32_t w[SLOTW];
+        read_slot(slot, w);
+        al[s] = ld_row<V, R>(facp[N - 1], w[N - 1]);
+        uint32_t f = w[N - 1] >> 31;
 #pragma unroll
-        for (int l = 0; l < NL; ++l) {
-            diff = diff || (nxt.k[l] != cur.k[l]);
-            e |= diff ? (1u << l) : 0u;
+        for (int l = 1; l < NL; ++l) {
+            if (w[l] & kFlag) rb[l][s] = ld_row<V, R>(facp[l], w[l]);
+            f |= (w[l] >> 31) << l;
         }
-        const float v = (!FUSED || j < n_real) ? cur.val : 0.f;      // padding records carry value 0
-        write_out(j, cur, v);
-        al[slot] = ld_row<V>(facp[N - 1], cur.k[N - 1], R);
-#pragma unroll
-        for (int l = 1; l < NL; ++l)
-            if (e & (1u << l)) rb[l][slot] = ld_row<V>(facp[l], cur.k[l], R);
-        val[slot] = v;
-        ef[slot] = e;
-        cur = nxt;
+        val[s] = __uint_as_float(w[N]);
+        fl[s] = f;
     };
-    // Arithmetic of step j (its record sits at `jslot`).
-    auto process = [&](int j, const uint32_t* jslot, int slot) {
-        const unsigned e = ef[slot];
-        vfmas<V>(t[NL - 1], val[slot], al[slot]);
+    // Arithmetic of one step (its record sits at `slot`).
+    auto compute = [&](const uint32_t* slot, int s) {
+        const uint32_t e = fl[s];
+        vfmas<V>(t[NL - 1], val[s], al[s]);
 #pragma unroll
         for (int l = NL - 1; l >= 1; --l) {
             if (e & (1u << l)) {
-                vfma<V>(t[l - 1], rb[l][slot], t[l]);
+                vfma<V>(t[l - 1], rb[l][s], t[l]);
                 t[l] = vzero<V>();
             }
         }
-        if ((e & 1u) && j + 1 < C) {                      // an output row ends inside the chunk
-            const uint32_t row = jslot[k0w];
-            float* dst = (seg == 0) ? &s_first[warp][g][sub * V] : a.out + (size_t)row * R + sub * V;
-            vstore<V>(dst, t[0]);
-            if (seg == 0 && sub == 0) s_erow[warp][2 * g] = (int)row;
+        if (e & 1u) {                                     // an output row ends inside the chunk
+            const uint32_t row = slot[0];
+            if (seg == 0) {
+                vstore<V>(&s_first[warp][g][sub * V], t[0]);
+                if (sub == 0) s_erow[warp][2 * g] = (int)row;
+            } else {
+                vstore<V>(a.out + (size_t)row * R + sub * V, t[0]);
+            }
             ++seg;
             t[0] = vzero<V>();
         }
     };
 
+    // ---- prologue: rounds 0..STAGES-2 in flight, rounds 0 (and 1) landed and fixed -----------------
+    constexpr int AHEAD = STAGES - 1;                     // rounds issued ahead of the one being computed
 #pragma unroll
-    for (int r = 0; r < STAGES - 1; ++r) {
-        load_prev(r, pvA);
-        issue_round(r, pvA);
+    for (int r = 0; r < AHEAD; ++r) {
+        load_prev(r);
+        issue_round(r);
     }
-    load_prev(STAGES - 1, pvA);
-    load_prev(STAGES, pvB);
-    cp_async_wait<STAGES - 2>();                          // round 0 has landed
+    load_prev(AHEAD);
+    cp_async_wait<AHEAD - 2>();                           // rounds 0 and 1 have landed
     __syncwarp();
-    cur = read_rec(ring_g);
-    lookahead(0, ring_g + 1 * ROWW, 0);
-    lookahead(1, ring_g + 2 * ROWW, 1);
-    for (int r = 0; r < nrounds; ++r) {
-        issue_round(r + STAGES - 1, pvA);
-        if constexpr (FUSED) {
+    fix_round(0);
+    __syncwarp();
 #pragma unroll
-            for (int i = 0; i < NPIECE; ++i) pvA[i] = pvB[i];
-            load_prev(r + STAGES + 1, pvB);
-        }
-        cp_async_wait<STAGES - 2>();                      // rounds <= r+1 have landed
+    for (int i = 0; i < D; ++i) prefetch(ring_g + i * ROWW, i);
+    for (int r = 0; r < nrounds; ++r) {
+        issue_round(r + AHEAD);                           // reuses the stage of round r-1
+        load_prev(r + AHEAD + 1);
+        cp_async_wait<AHEAD - 2>();                       // rounds <= r+2 have landed
         __syncwarp();
-        const uint32_t* cs = ring_g + (r & (STAGES - 1)) * STAGEW;          // this round's stage
-        const uint32_t* ns = ring_g + ((r + 1) & (STAGES - 1)) * STAGEW;    // next round's stage
-        const int j0 = r * K;
+        fix_round(r + 1);
+        __syncwarp();
+        const uint32_t* cs = ring_g + (r % STAGES) * STAGEW;            // this round's stage
+        const uint32_t* ns = ring_g + ((r + 1) % STAGES) * STAGEW;      // next round's stage
         const bool more = r + 1 < nrounds;
-        process(j0 + 0, cs + 0 * ROWW, 0);
-        lookahead(j0 + 2, cs + 3 * ROWW, 0);
-        process(j0 + 1, cs + 1 * ROWW, 1);
-        lookahead(j0 + 3, ns + 0 * ROWW, 1);
-        process(j0 + 2, cs + 2 * ROWW, 0);
-        if (more) lookahead(j0 + 4, ns + 1 * ROWW, 0);
-        process(j0 + 3, cs + 3 * ROWW, 1);
-        if (more) lookahead(j0 + 5, ns + 2 * ROWW, 1);
+#pragma unroll
+        for (int i = 0; i < K; ++i) {
+            compute(cs + i * ROWW, i % D);
+            if (i + D < K) prefetch(cs + (i + D) * ROWW, i % D);
+            else if (more) prefetch(ns + (i + D - K) * ROWW, i % D);
+        }
         __syncwarp();                                     // everyone is done with round r's stage
     }
     cp_async_wait<0>();
-    const uint32_t last_row = ring_g[((C - 1) & (STAGES * K - 1)) * ROWW + k0w];
+    uint32_t lastw[SLOTW];
+    read_slot(ring_g + ((nrounds - 1) % STAGES) * STAGEW + (K - 1) * ROWW, lastw);
+    const uint32_t last_row = lastw[0];
     __syncwarp();
     // chunk epilogue: the still-open row goes to the first (seg == 0) or last partial-row entry
     float* const s_last = reinterpret_cast<float*>(ring);               // [NPW][R], aliases the ring
@@ -451,8 +500,8 @@ __global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a)
         // because the neighbouring shards may not have written T_out yet)
         auto key0_at = [&](int64_t pos) {
             if constexpr (FUSED) {
-                if (pos > a.nnz_real - 1) pos = a.nnz_real - 1;
-                return __ldg(a.rec + (size_t)__ldg(a.prev + pos) * RECW + a.src[0]);
+                if (pos > fa.nnz_real - 1) pos = fa.nnz_real - 1;
+                return __ldg(a.rec + (size_t)__ldg(fa.prev + pos) * RECW + fa.src[0]);
             } else {
                 return __ldg(a.rec + (size_t)pos * RECW);
             }
@@ -514,15 +563,16 @@ __global__ void __launch_bounds__(256) k_zero_rows(const uint32_t* __restrict__ 
 }
 
 template <int N, int R, bool FUSED>
-static mttkrp_status_t launch_main(const KernelArgs<N>& a, int64_t num_shards, Timing* timing, cudaStream_t st) {
-    constexpr int smem = Geo<N, R>::SMEM_BYTES;
+static mttkrp_status_t launch_main(const KernelArgs<N>& a, const FuseArgs<N>& fa, int64_t num_shards, Timing* timing,
+                                   cudaStream_t st) {
+    constexpr int smem = Geo<N, R, FUSED>::SMEM_BYTES;
     static bool attr_set = false;
     if (!attr_set) {
         MK_CUDA(cudaFuncSetAttribute(k_mttkrp<N, R, FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         attr_set = true;
     }
     TimedLaunch tl(timing, kClsMttkrp, st);
-    k_mttkrp<N, R, FUSED><<<(unsigned)num_shards, kBlockThreads, smem, st>>>(a);
+    k_mttkrp<N, R, FUSED><<<(unsigned)num_shards, kBlockThreads, smem, st>>>(a, fa);
     return MTTKRP_OK;
 }
 
@@ -546,26 +596,27 @@ static mttkrp_status_t launch_nr(mttkrp_handle_s* h, int d, const float* const* 
         for (int l = 1; l < N; ++l) a.fac[l] = factors[mm.order[l]];
         a.out = out;
         a.carry = h->carry;
-        a.prev = nullptr;
-        a.rec_out = nullptr;
-        a.nnz_real = h->nnz;
-        a.dpos_packed = 0;
-        for (int l = 0; l < N; ++l) { a.src[l] = l; a.dpos_packed |= (uint32_t)l << (4 * l); }
+        FuseArgs<N> fa;
+        fa.prev = nullptr;
+        fa.rec_out = nullptr;
+        fa.nnz_real = h->nnz;
+        fa.dpos_packed = 0;
+        for (int l = 0; l < N; ++l) { fa.src[l] = l; fa.dpos_packed |= (uint32_t)l << (4 * l); }
         if (fuse_from >= 0) {
             // remap fuse_from -> d inside the MTTKRP kernel; T_out becomes the resident copy
-            a.prev = h->mode[fuse_from].next;
-            a.rec_out = h->rec_alt;
-            for (int l = 0; l < N; ++l) a.src[l] = h->mode[fuse_from].pos[mm.order[l]];
-            a.dpos_packed = 0;
-            for (int l = 0; l < N; ++l) a.dpos_packed |= (uint32_t)l << (4 * a.src[l]);
-            MK_TRY((launch_main<N, R, true>(a, h->num_shards, h->timing, st)));
+            fa.prev = h->mode[fuse_from].next;
+            fa.rec_out = h->rec_alt;
+            for (int l = 0; l < N; ++l) fa.src[l] = h->mode[fuse_from].pos[mm.order[l]];
+            fa.dpos_packed = 0;
+            for (int l = 0; l < N; ++l) fa.dpos_packed |= (uint32_t)l << (4 * fa.src[l]);
+            MK_TRY((launch_main<N, R, true>(a, fa, h->num_shards, h->timing, st)));
             uint32_t* t = h->rec_cur;      // swap(T_in, T_out), Alg. 5 line 12
             h->rec_cur = h->rec_alt;
             h->rec_alt = t;
             h->cur = d;
             h->remaps_done++;
         } else {
-            MK_TRY((launch_main<N, R, false>(a, h->num_shards, h->timing, st)));
+            MK_TRY((launch_main<N, R, false>(a, fa, h->num_shards, h->timing, st)));
         }
         if (mm.n_chains > 0) {
             TimedLaunch tl(h->timing, kClsFixup, st);
