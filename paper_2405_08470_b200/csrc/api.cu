@@ -47,16 +47,11 @@ static mttkrp_status_t ensure_layout(mttkrp_handle_s* h, int d, cudaStream_t st)
     return MTTKRP_OK;
 }
 
-// Mode d on whatever layout is resident: separate remap passes until the copy is one step before
-// d, then the last step fused into the MTTKRP kernel (Alg. 4); the cyclic order
-// of Alg. 5 therefore runs one kernel per mode.
+// Mode d on whatever layout is resident: remap passes until the copy is in layout d (the cyclic
+// order of Alg. 5 costs one), then the MTTKRP kernels.
 static mttkrp_status_t run_mode(mttkrp_handle_s* h, int d, const float* const* factors, int R, float* out, cudaStream_t st) {
-    if (h->cur == d || !h->fuse || h->nnz == 0) {
-        MK_TRY(ensure_layout(h, d, st));
-        return launch_mttkrp(h, d, factors, R, out, -1, st);
-    }
-    MK_TRY(ensure_layout(h, (d + h->N - 1) % h->N, st));
-    return launch_mttkrp(h, d, factors, R, out, h->cur, st);
+    MK_TRY(ensure_layout(h, d, st));
+    return launch_mttkrp(h, d, factors, R, out, st);
 }
 
 }  // namespace mk
@@ -116,13 +111,6 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
     h->max_rank = max_rank;
     h->device = dev;
     h->timing = new (std::nothrow) Timing();
-    {
-        // MTTKRP_FUSE=1: do the last remap step inside the MTTKRP kernel (the paper's Alg. 4 design).
-        // Off by default: on B200 the separate gather pass + lean MTTKRP kernel measured faster on 4 of
-        // the 5 configs.
-        const char* env = getenv("MTTKRP_FUSE");
-        h->fuse = (env && env[0] == '1') ? 1 : 0;
-    }
     for (int d = 0; d < nmodes; ++d) {
         ModeMeta& mm = h->mode[d];
         choose_key_order(nmodes, dims, d, mm.order);

@@ -268,15 +268,29 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_scatter(const uint32_t* 
 // rec[k] = { idx[order[0]][perm[k]], ..., idx[order[N-1]][perm[k]], val[perm[k]] }
 struct OrderArg { int v[kMaxModes]; };
 
-// Positions k in [nnz, nnz_pad) are padding: the keys of the last nonzero with value 0.
+// Positions k in [nnz, nnz_pad) are padding: the keys of the last nonzero with value 0.  Bit 31 of
+// the key words gets the run-end flags (common.cuh), from the keys of the record at k+1.
 __global__ void k_build_records(const int32_t* __restrict__ idx, const float* __restrict__ vals,
                                 const uint32_t* __restrict__ perm, int64_t nnz, int64_t nnz_pad, int N, OrderArg order,
                                 uint32_t* __restrict__ rec) {
     int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= nnz_pad) return;
-    uint32_t src = perm[k < nnz ? k : nnz - 1];
+    const uint32_t src = perm[k < nnz ? k : nnz - 1];
+    const bool last = k + 1 >= nnz_pad;
+    const uint32_t nsrc = last ? src : perm[k + 1 < nnz ? k + 1 : nnz - 1];
     uint32_t* r = rec + (size_t)k * (N + 1);
-    for (int l = 0; l < N; ++l) r[l] = (uint32_t)idx[(size_t)order.v[l] * nnz + src];
+    bool diff = last, e0 = false;
+    for (int l = 0; l < N; ++l) {
+        const uint32_t key = (uint32_t)idx[(size_t)order.v[l] * nnz + src];
+        uint32_t flag = 0u;
+        if (l < N - 1) {
+            diff = diff || ((uint32_t)idx[(size_t)order.v[l] * nnz + nsrc] != key);
+            if (l == 0) e0 = diff;
+            else flag = diff ? kFlag : 0u;
+        }
+        if (l == N - 1) flag = e0 ? kFlag : 0u;
+        r[l] = key | (l == 0 ? 0u : flag);
+    }
     r[N] = k < nnz ? __float_as_uint(vals[src]) : 0u;
 }
 

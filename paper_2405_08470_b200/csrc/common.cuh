@@ -31,6 +31,29 @@ void set_error(const char* fmt, ...);
         if (s__ != MTTKRP_OK) return s__;         \
     } while (0)
 
+// Run-end flags.  A record of the mode-d layout is N uint32 key words (k_0 = i_d first) + the fp32
+// value.  Indices are < 2^31, so bit 31 of a key word is free; the format builder and the remap pass
+// store there, for the record at position j, e_l = "record j+1 differs from record j in one of the
+// keys k_0..k_l" (the run of equal (k_0..k_l) ends at j):  e_l sits in word l for 1 <= l <= N-2 and
+// e_0 (the output row ends) in word N-1.  Word 0 is never flagged.  Padding records repeat the keys of
+// the last nonzero (no run ends); the very last record of the padded array has every flag set.
+constexpr uint32_t kFlag = 0x80000000u;
+constexpr uint32_t kKeyMask = 0x7fffffffu;
+
+// flags of a record from its keys `k` and the keys `nk` of the record after it (sorted order)
+template <int N>
+__device__ __forceinline__ void set_run_flags(uint32_t* k, const uint32_t* nk, bool last_of_array) {
+    bool diff = last_of_array;
+    bool e0 = false;
+#pragma unroll
+    for (int l = 0; l < N - 1; ++l) {
+        diff = diff || (nk[l] != k[l]);
+        if (l == 0) e0 = diff;
+        else k[l] |= diff ? kFlag : 0u;
+    }
+    k[N - 1] |= e0 ? kFlag : 0u;
+}
+
 // Per-mode tables built by mttkrp_create.
 struct ModeMeta {
     int order[kMaxModes];     // sort-key order of this layout, order[0] == mode
@@ -89,7 +112,6 @@ struct mttkrp_handle_s {
     int64_t bytes_held;
     int64_t remaps_done;
     int device;
-    int fuse;                 // 1: last remap step inside the MTTKRP kernel (opt-in, MTTKRP_FUSE=1)
     mk::Timing* timing;       // owned; per-kernel event pairs while mttkrp_timing_begin is active
 };
 
@@ -117,6 +139,6 @@ mttkrp_status_t launch_perm_step(const uint32_t* map, const uint32_t* in, uint32
 
 // ---- mttkrp_kernel.cu -----------------------------------------------------------------------
 mttkrp_status_t launch_mttkrp(mttkrp_handle_s* h, int d, const float* const* factors, int R,
-                              float* out, int fuse_from, cudaStream_t st);
+                              float* out, cudaStream_t st);
 
 }  // namespace mk

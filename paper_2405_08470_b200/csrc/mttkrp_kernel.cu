@@ -3,22 +3,25 @@
 // library's own, made for sm_100a).
 //
 // Layout: records sorted by the key tuple (k_0 = i_d, k_1, ..., k_{N-1}); record = N uint32 keys in
-// that order + fp32 value.  In shared memory bit 31 of the key words carries the run-end flags, which a
-// per-stage fix-up pass derives from the sorted order once per record, so in the hot loop a record is
-// self-contained: no look-ahead compare in the hot loop.
+// that order + fp32 value.  Bit 31 of the key words carries the run-end flags that the format builder
+// and the remap pass derived from the sorted order (common.cuh), so a record is self-contained: the
+// hot loop has no look-ahead compare.
 // A thread block owns one shard = shard_nnz consecutive records (equal-nnz shards).  Inside the
-// block a GROUP of R/V lanes (V = 8 rank columns per lane, one 256-bit LDG per factor row per lane)
-// walks a contiguous chunk of the shard one nonzero at a time:
+// block a GROUP of R/V lanes (V = 4 rank columns per lane, one 128-bit LDG per factor row per lane:
+// a warp instruction then covers whole 128-byte lines, one L1 wavefront each) walks a contiguous
+// chunk of the shard one nonzero at a time:
 //   l(r) = val * prod_w A_w[i_w, r]         (Alg. 2 lines 8-13)
 //   Y_d[i_d, r] += l(r)                     (Alg. 2 lines 14-15)
 // Because the chunk is sorted, the products are nested sums (a CSF-style factoring of the same
 // expression):  Y[k_0] = sum_{k_1} A[k_1] * ( sum_{k_2} A[k_2] * ( ... sum_{k_{N-1}} val * A[k_{N-1}] ) ),
 // so the row of level l is gathered once per run of equal (k_0..k_l), at the END of the run.
 //
-// Pipeline per warp: records are staged into a shared-memory ring with cp.async (4-6 stages of K
+// Pipeline per warp: records are staged into a shared-memory ring with cp.async (stages of K
 // records per group, interleaved by group so one LDS.128 serves all groups without bank conflicts).
 // D steps ahead of the arithmetic the group reads its record from the ring and issues the
 // factor-row gathers for that step into rotating registers.  The arithmetic is packed fp32x2 FMA.
+// The kernel is bound by the L1 data pipe (one wavefront per gathered line), so every other use of
+// that pipe is kept minimal: one cp.async and one LDS per record.
 //
 // Rows that begin and end inside a chunk are stored with plain stores by their only owner
 // (Observation 2: no global atomics).  The first/last partial rows of each chunk
@@ -122,24 +125,35 @@ template <int NPEND>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(NPEND) : "memory"); }
 
 // ---- compile-time geometry ---------------------------------------------------------------------
-template <int N, int R, bool FUSED>
+#ifndef MK_V8
+#define MK_V8 0          // 1: 8 columns per lane (256-bit gathers); measured 1.4 L1 wavefronts per 128-byte line
+#endif                   //    against 1.0 for 128-bit gathers (profiles/r1_probe_gather.md)
+#ifndef MK_D
+#define MK_D 2
+#endif
+#ifndef MK_STAGES
+#define MK_STAGES 3
+#endif
+#ifndef MK_MINB          // resident blocks per SM the register allocation must allow; 0 = per-N default below.
+#define MK_MINB 0        // Measured on B200 (configs[1], configs[2]): occupancy beats deeper look-ahead.
+#endif
+template <int N, int R>
 struct Geo {
-    static constexpr int V = (R >= 16) ? 8 : 4;          // rank columns per lane
+    static constexpr int V = (MK_V8 && R >= 16) ? 8 : 4; // rank columns per lane
     static constexpr int LPN = R / V;                    // lanes per nonzero (group size)
     static constexpr int NPW = 32 / LPN;                 // groups per warp
     static constexpr int WARPS = kBlockThreads / 32;
     static constexpr int G = WARPS * NPW;                // groups per block
     static constexpr int RECW = N + 1;                   // record words
     static constexpr int SLOTW = (RECW + 3) / 4 * 4;     // ring slot words (16-byte multiple)
-    static constexpr int K = (NPW * SLOTW <= 32 || NPW < 8) ? 8 : 4;  // records per group per ring stage
-    // ring stages: round r computing, r+1 fixed up, r+2 landed, the rest in flight (the fused variant
-    // gathers records from random DRAM positions and keeps more rounds in flight)
-    static constexpr int STAGES = (FUSED && K * NPW * SLOTW * 4 <= 1024) ? 6 : 4;
-    static constexpr int D = 2;                          // gather look-ahead, in steps (K % D == 0)
+    static constexpr int K = (NPW * SLOTW <= 32) ? 8 : 4;  // records per group per ring stage
+    static constexpr int STAGES = MK_STAGES;             // round r computing, r+1 landed, the rest in flight
+    static constexpr int D = (MK_D < K) ? MK_D : K / 2;  // gather look-ahead, in steps (K % D == 0)
     static constexpr int RING_WORDS = STAGES * K * NPW * SLOTW;        // per warp
     static constexpr int ENT_WORDS = 2 * NPW * R;                       // per warp: first/last partial rows
     static constexpr int WARP_WORDS = RING_WORDS > ENT_WORDS ? RING_WORDS : ENT_WORDS;
     static constexpr int NL = N - 1;                     // accumulator levels t[0..NL-1]
+    static constexpr int MINB = MK_MINB ? MK_MINB : (N <= 3 ? 5 : 3);
     static constexpr int SMEM_BYTES = 4 * (WARPS * WARP_WORDS + WARPS * NPW * R + 2 * WARPS * R + WARPS * 2 * NPW + 2 * WARPS);
 };
 
@@ -170,37 +184,19 @@ __device__ __forceinline__ void merge_runs(const int* rows, const float* vecs, i
     if (cur_row >= 0) emit(cur_row, acc, run == 0, true);
 }
 
-constexpr uint32_t kFlag = 0x80000000u;   // run-end flag bit inside a key word (shared memory only)
-
-// FUSED = false: `rec` is the tensor copy already in this mode's layout (after a separate remap pass).
-// FUSED = true : dynamic remapping inside the kernel (Alg. 4 lines 17-19: elementwise
-//   computation and dynamic remapping in one kernel).  `rec` is T_in in the PREVIOUS layout; record j of
-//   this layout is T_in[prev[j]] with its index fields permuted (field l <- source field src[l]); the
-//   kernel gathers it straight into the shared-memory ring with cp.async and also writes it to
-//   rec_out[j] (T_out, this layout), which is the next mode's T_in.
-template <int N>
-struct FuseArgs {
-    const uint32_t* prev;    // [nnz_real] gather map
-    uint32_t* rec_out;       // padded like rec
-    int64_t nnz_real;
-    int src[N];
-    uint32_t dpos_packed;    // 4 bits per source field: its level in this layout
-};
-
-template <int N, int R, bool FUSED>
-__global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a, const FuseArgs<N> fa) {
-    using Ge = Geo<N, R, FUSED>;
+template <int N, int R>
+__global__ void __launch_bounds__(kBlockThreads, Geo<N, R>::MINB) k_mttkrp(const KernelArgs<N> a) {
+    using Ge = Geo<N, R>;
     constexpr int V = Ge::V, LPN = Ge::LPN, NPW = Ge::NPW, WARPS = Ge::WARPS, G = Ge::G, K = Ge::K, D = Ge::D;
     constexpr int STAGES = Ge::STAGES, RECW = Ge::RECW, SLOTW = Ge::SLOTW, NL = Ge::NL;
     constexpr int ROWW = NPW * SLOTW;                     // ring words between consecutive records of a group
     constexpr int STAGEW = K * ROWW;                      // ring words per stage
-    constexpr int RPL = K * NPW / 32;                     // records per lane per stage in the fix-up pass
-    // cp.async piece: the widest power of two dividing the record; the fused variant permutes the
-    // index fields for free at copy time with 4-byte pieces, and with selects for 16-byte records.
-    constexpr int PW = FUSED ? (N == 3 ? 4 : 1) : (RECW % 4 == 0 ? 4 : (RECW % 2 == 0 ? 2 : 1));
+    // cp.async piece: the widest power of two (4, 8 or 16 bytes) dividing the record
+    constexpr int PW = RECW % 4 == 0 ? 4 : (RECW % 2 == 0 ? 2 : 1);
     constexpr int PPR = RECW / PW;                        // pieces per record
     constexpr int NPIECE = (K * PPR + LPN - 1) / LPN;     // pieces per lane per round
-    static_assert(K % D == 0 && RPL >= 1 && K * NPW % 32 == 0, "geometry");
+    constexpr int AHEAD = STAGES - 1;                     // rounds issued ahead of the one being computed
+    static_assert(K % D == 0 && D < K && STAGES >= 3, "geometry");
 
     extern __shared__ uint4 smem_raw[];
     // carve-up (Geo::SMEM_BYTES): record rings (later the groups' last partial rows) | the groups'
@@ -218,49 +214,28 @@ __global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a,
     // so every chunk holds exactly C records and the loop needs no bounds checks.
     const int64_t s_begin = shard * (int64_t)a.shard_nnz;
     const int64_t s_end = s_begin + a.shard_nnz;
-    const int C = a.shard_nnz / G;                        // records per group; a multiple of K
+    const int C = a.shard_nnz / G;                        // records per group; a multiple of K, > D
     const int nrounds = C / K;
-    const int64_t wb = s_begin + (int64_t)(warp * NPW) * C;             // first position of this warp's groups
-    const int64_t cb = wb + (int64_t)g * C;                             // this group's first position
+    const int64_t cb = s_begin + (int64_t)(warp * NPW + g) * C;         // this group's first position
+    const uint32_t* const grec = a.rec + (size_t)cb * RECW;
 
     uint32_t* const ring = &s_warp[warp][0];
-    uint32_t* const ring_g = ring + g * SLOTW;            // this group's column of the ring
+    const uint32_t* const ring_g = ring + g * SLOTW;      // this group's column of the ring
     const uint32_t ring_gs = (uint32_t)__cvta_generic_to_shared(ring_g);
 
-    // ---- record staging -------------------------------------------------------------------------
-    // fused: source positions of this lane's pieces, fetched one round before they are needed
-    uint32_t pv[NPIECE];
-    auto load_prev = [&](int r) {
-        if constexpr (FUSED) {
-#pragma unroll
-            for (int i = 0; i < NPIECE; ++i) {
-                const int p = sub + i * LPN;
-                const int jj = p / PPR;
-                int64_t j = cb + (int64_t)r * K + jj;
-                if (j > fa.nnz_real - 1) j = fa.nnz_real - 1;        // padding copies the last nonzero
-                pv[i] = (p < K * PPR && r < nrounds) ? __ldcs(fa.prev + j) : 0u;
-            }
-        }
-    };
     auto issue_round = [&](int r) {
         if (r < nrounds) {
-            const uint32_t* src = a.rec + (size_t)(cb + (int64_t)r * K) * RECW;
+            const uint32_t* src = grec + (size_t)r * (K * RECW);
             const uint32_t dst = ring_gs + 4u * (uint32_t)((r % STAGES) * STAGEW);
 #pragma unroll
             for (int i = 0; i < NPIECE; ++i) {
                 const int p = sub + i * LPN;
                 if (p < K * PPR) {
                     const int jj = p / PPR, q = p % PPR;
-                    if constexpr (FUSED) {
-                        const uint32_t* s2 = a.rec + (size_t)pv[i] * RECW + q * PW;
-                        if constexpr (PW == 4) cp_async16(dst + 4u * (uint32_t)(jj * ROWW), s2);
-                        else cp_async4(dst + 4u * (uint32_t)(jj * ROWW + (q < N ? (int)((fa.dpos_packed >> (4 * q)) & 15u) : N)), s2);
-                    } else {
-                        const uint32_t d2 = dst + 4u * (uint32_t)(jj * ROWW + q * PW);
-                        if constexpr (PW == 4) cp_async16(d2, src + jj * RECW + q * PW);
-                        else if constexpr (PW == 2) cp_async8(d2, src + jj * RECW + q * PW);
-                        else cp_async4(d2, src + jj * RECW + q * PW);
-                    }
+                    const uint32_t d2 = dst + 4u * (uint32_t)(jj * ROWW + q * PW);
+                    if constexpr (PW == 4) cp_async16(d2, src + jj * RECW + q * PW);
+                    else if constexpr (PW == 2) cp_async8(d2, src + jj * RECW + q * PW);
+                    else cp_async4(d2, src + jj * RECW + q * PW);
                 }
             }
         }
@@ -272,83 +247,6 @@ __global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a,
         for (int i = 0; i < SLOTW / 4; ++i) {
             const uint4 v = p[i];
             w[4 * i] = v.x; w[4 * i + 1] = v.y; w[4 * i + 2] = v.z; w[4 * i + 3] = v.w;
-        }
-    };
-    // Fix-up pass over stage r (all of it has landed, and so has record 0 of stage r+1): every lane
-    // takes RPL records, puts the keys into this layout's order (fused), derives the run-end flags
-    // from the following record of the same group and stores them in bit 31 of the key words
-    // (flag e_l in word l for 1 <= l <= N-2, e_0 in word N-1), and (fused) writes the record to T_out.
-    // The chunk's last record closes every inner run and leaves the output row open (epilogue).
-    auto fix_round = [&](int r) {
-        if (r >= nrounds) return;
-        uint32_t* const st = ring + (r % STAGES) * STAGEW;
-        const uint32_t* const stn = ring + ((r + 1) % STAGES) * STAGEW;
-#pragma unroll
-        for (int i = 0; i < RPL; ++i) {
-            const int q = lane + 32 * i;
-            const int jj = q / NPW, gg = q % NPW;
-            uint32_t* slot = st + jj * ROWW + gg * SLOTW;
-            const uint32_t* nslot = (jj + 1 < K) ? slot + ROWW : stn + gg * SLOTW;
-            uint32_t w[SLOTW], nx[SLOTW];
-            read_slot(slot, w);
-            read_slot(nslot, nx);                          // stale past the chunk end; masked by `last`
-            __syncwarp();                                  // every lane has read before any slot is rewritten
-            uint32_t k[N], nk[N];
-            if constexpr (FUSED && N == 3) {               // permute the index fields (uniform selects)
-#pragma unroll
-                for (int l = 0; l < 3; ++l) {
-                    k[l] = fa.src[l] == 0 ? w[0] : (fa.src[l] == 1 ? w[1] : w[2]);
-                    nk[l] = fa.src[l] == 0 ? nx[0] : (fa.src[l] == 1 ? nx[1] : nx[2]);
-                }
-            } else {
-#pragma unroll
-                for (int l = 0; l < N; ++l) { k[l] = w[l]; nk[l] = nx[l]; }
-            }
-            uint32_t val = w[N];
-            const bool last = (r == nrounds - 1) && (jj == K - 1);
-            const int64_t pos = wb + (int64_t)gg * C + (int64_t)r * K + jj;
-            if constexpr (FUSED) {
-                if (pos >= fa.nnz_real) val = 0u;          // padding records carry value 0
-                uint32_t* o = fa.rec_out + (size_t)pos * RECW;
-                if constexpr (RECW % 4 == 0) {
-                    uint32_t ww[RECW];
-#pragma unroll
-                    for (int l = 0; l < N; ++l) ww[l] = k[l];
-                    ww[N] = val;
-#pragma unroll
-                    for (int c4 = 0; c4 < RECW / 4; ++c4)
-                        __stcs(reinterpret_cast<uint4*>(o) + c4, make_uint4(ww[4 * c4], ww[4 * c4 + 1], ww[4 * c4 + 2], ww[4 * c4 + 3]));
-                } else if constexpr (RECW % 2 == 0) {
-                    uint32_t ww[RECW];
-#pragma unroll
-                    for (int l = 0; l < N; ++l) ww[l] = k[l];
-                    ww[N] = val;
-#pragma unroll
-                    for (int c2 = 0; c2 < RECW / 2; ++c2) __stcs(reinterpret_cast<uint2*>(o) + c2, make_uint2(ww[2 * c2], ww[2 * c2 + 1]));
-                } else {
-#pragma unroll
-                    for (int l = 0; l < N; ++l) __stcs(o + l, k[l]);
-                    __stcs(o + N, val);
-                }
-            }
-            bool diff = false;
-            uint32_t o4[SLOTW];
-#pragma unroll
-            for (int l = 0; l < SLOTW; ++l) o4[l] = 0u;
-            o4[0] = k[0];
-            bool e0 = false;
-#pragma unroll
-            for (int l = 0; l < NL; ++l) {
-                diff = diff || (nk[l] != k[l]);
-                const bool e = last ? (l > 0) : diff;
-                if (l == 0) e0 = e;
-                else o4[l] = k[l] | (e ? kFlag : 0u);
-            }
-            o4[N - 1] = k[N - 1] | (e0 ? kFlag : 0u);
-            o4[N] = val;
-#pragma unroll
-            for (int c4 = 0; c4 < SLOTW / 4; ++c4)
-                reinterpret_cast<uint4*>(slot)[c4] = make_uint4(o4[4 * c4], o4[4 * c4 + 1], o4[4 * c4 + 2], o4[4 * c4 + 3]);
         }
     };
 
@@ -366,10 +264,17 @@ __global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a,
     uint32_t fl[D];                                       // bit l: the run of level l ends at this step
     int seg = 0;                                          // output-row segments finished in this chunk
 
-    // Issue the gathers of one step whose (fixed-up) record sits at `slot`.
-    auto prefetch = [&](const uint32_t* slot, int s) {
+    // Issue the gathers of one step whose record sits at `slot`.  The record carries its run-end
+    // flags (common.cuh).  The chunk's last record closes every inner run and leaves the output row
+    // open: it is finished by the epilogue, which knows whether the row continues in the next chunk.
+    auto prefetch = [&](const uint32_t* slot, int s, bool chunk_last) {
         uint32_t w[SLOTW];
         read_slot(slot, w);
+        if (chunk_last) {
+#pragma unroll
+            for (int l = 1; l < NL; ++l) w[l] |= kFlag;
+            w[N - 1] &= kKeyMask;
+        }
         al[s] = ld_row<V, R>(facp[N - 1], w[N - 1]);
         uint32_t f = w[N - 1] >> 31;
 #pragma unroll
@@ -404,26 +309,16 @@ __global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a,
         }
     };
 
-    // ---- prologue: rounds 0..STAGES-2 in flight, rounds 0 (and 1) landed and fixed -----------------
-    constexpr int AHEAD = STAGES - 1;                     // rounds issued ahead of the one being computed
+    // ---- prologue: rounds 0..AHEAD-1 in flight, round 0 landed ----------------------------------------
 #pragma unroll
-    for (int r = 0; r < AHEAD; ++r) {
-        load_prev(r);
-        issue_round(r);
-    }
-    load_prev(AHEAD);
-    cp_async_wait<AHEAD - 2>();                           // rounds 0 and 1 have landed
-    __syncwarp();
-    fix_round(0);
+    for (int r = 0; r < AHEAD; ++r) issue_round(r);
+    cp_async_wait<AHEAD - 1>();                           // round 0 has landed
     __syncwarp();
 #pragma unroll
-    for (int i = 0; i < D; ++i) prefetch(ring_g + i * ROWW, i);
+    for (int i = 0; i < D; ++i) prefetch(ring_g + i * ROWW, i, false);
     for (int r = 0; r < nrounds; ++r) {
         issue_round(r + AHEAD);                           // reuses the stage of round r-1
-        load_prev(r + AHEAD + 1);
-        cp_async_wait<AHEAD - 2>();                       // rounds <= r+2 have landed
-        __syncwarp();
-        fix_round(r + 1);
+        cp_async_wait<AHEAD - 1>();                       // rounds <= r+1 have landed
         __syncwarp();
         const uint32_t* cs = ring_g + (r % STAGES) * STAGEW;            // this round's stage
         const uint32_t* ns = ring_g + ((r + 1) % STAGES) * STAGEW;      // next round's stage
@@ -431,15 +326,13 @@ __global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a,
 #pragma unroll
         for (int i = 0; i < K; ++i) {
             compute(cs + i * ROWW, i % D);
-            if (i + D < K) prefetch(cs + (i + D) * ROWW, i % D);
-            else if (more) prefetch(ns + (i + D - K) * ROWW, i % D);
+            if (i + D < K) prefetch(cs + (i + D) * ROWW, i % D, (i + D == K - 1) && !more);
+            else if (more) prefetch(ns + (i + D - K) * ROWW, i % D, false);
         }
         __syncwarp();                                     // everyone is done with round r's stage
     }
     cp_async_wait<0>();
-    uint32_t lastw[SLOTW];
-    read_slot(ring_g + ((nrounds - 1) % STAGES) * STAGEW + (K - 1) * ROWW, lastw);
-    const uint32_t last_row = lastw[0];
+    const uint32_t last_row = ring_g[((nrounds - 1) % STAGES) * STAGEW + (K - 1) * ROWW];
     __syncwarp();
     // chunk epilogue: the still-open row goes to the first (seg == 0) or last partial-row entry
     float* const s_last = reinterpret_cast<float*>(ring);               // [NPW][R], aliases the ring
@@ -496,16 +389,7 @@ __global__ void __launch_bounds__(kBlockThreads) k_mttkrp(const KernelArgs<N> a,
 
     // level 2: merge the warps' partial rows; rows shared with a neighbouring shard go to the carry buffer
     if (warp == 0) {
-        // output index of the record at position pos of THIS layout (fused: through the gather map,
-        // because the neighbouring shards may not have written T_out yet)
-        auto key0_at = [&](int64_t pos) {
-            if constexpr (FUSED) {
-                if (pos > fa.nnz_real - 1) pos = fa.nnz_real - 1;
-                return __ldg(a.rec + (size_t)__ldg(fa.prev + pos) * RECW + fa.src[0]);
-            } else {
-                return __ldg(a.rec + (size_t)pos * RECW);
-            }
-        };
+        auto key0_at = [&](int64_t pos) { return __ldg(a.rec + (size_t)pos * RECW); };   // word 0 carries no flag
         const uint32_t first_row = key0_at(s_begin);
         const uint32_t end_row = key0_at(s_end - 1);
         const bool head_shared = s_begin > 0 && key0_at(s_begin - 1) == first_row;
@@ -562,23 +446,8 @@ __global__ void __launch_bounds__(256) k_zero_rows(const uint32_t* __restrict__ 
         *(reinterpret_cast<float4*>(out + (size_t)rows[i] * R) + sub) = make_float4(0.f, 0.f, 0.f, 0.f);
 }
 
-template <int N, int R, bool FUSED>
-static mttkrp_status_t launch_main(const KernelArgs<N>& a, const FuseArgs<N>& fa, int64_t num_shards, Timing* timing,
-                                   cudaStream_t st) {
-    constexpr int smem = Geo<N, R, FUSED>::SMEM_BYTES;
-    static bool attr_set = false;
-    if (!attr_set) {
-        MK_CUDA(cudaFuncSetAttribute(k_mttkrp<N, R, FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        attr_set = true;
-    }
-    TimedLaunch tl(timing, kClsMttkrp, st);
-    k_mttkrp<N, R, FUSED><<<(unsigned)num_shards, kBlockThreads, smem, st>>>(a, fa);
-    return MTTKRP_OK;
-}
-
 template <int N, int R>
-static mttkrp_status_t launch_nr(mttkrp_handle_s* h, int d, const float* const* factors, float* out, int fuse_from,
-                                 cudaStream_t st) {
+static mttkrp_status_t launch_nr(mttkrp_handle_s* h, int d, const float* const* factors, float* out, cudaStream_t st) {
     const ModeMeta& mm = h->mode[d];
     if (mm.n_empty > 0) {
         const int64_t groups = mm.n_empty;
@@ -596,65 +465,47 @@ static mttkrp_status_t launch_nr(mttkrp_handle_s* h, int d, const float* const* 
         for (int l = 1; l < N; ++l) a.fac[l] = factors[mm.order[l]];
         a.out = out;
         a.carry = h->carry;
-        FuseArgs<N> fa;
-        fa.prev = nullptr;
-        fa.rec_out = nullptr;
-        fa.nnz_real = h->nnz;
-        fa.dpos_packed = 0;
-        for (int l = 0; l < N; ++l) { fa.src[l] = l; fa.dpos_packed |= (uint32_t)l << (4 * l); }
-        if (fuse_from >= 0) {
-            // remap fuse_from -> d inside the MTTKRP kernel; T_out becomes the resident copy
-            fa.prev = h->mode[fuse_from].next;
-            fa.rec_out = h->rec_alt;
-            for (int l = 0; l < N; ++l) fa.src[l] = h->mode[fuse_from].pos[mm.order[l]];
-            fa.dpos_packed = 0;
-            for (int l = 0; l < N; ++l) fa.dpos_packed |= (uint32_t)l << (4 * fa.src[l]);
-            MK_TRY((launch_main<N, R, true>(a, fa, h->num_shards, h->timing, st)));
-            uint32_t* t = h->rec_cur;      // swap(T_in, T_out), Alg. 5 line 12
-            h->rec_cur = h->rec_alt;
-            h->rec_alt = t;
-            h->cur = d;
-            h->remaps_done++;
-        } else {
-            MK_TRY((launch_main<N, R, false>(a, fa, h->num_shards, h->timing, st)));
+        constexpr int smem = Geo<N, R>::SMEM_BYTES;
+        static bool attr_set = false;
+        if (!attr_set) {
+            MK_CUDA(cudaFuncSetAttribute(k_mttkrp<N, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            attr_set = true;
+        }
+        {
+            TimedLaunch tl(h->timing, kClsMttkrp, st);
+            k_mttkrp<N, R><<<(unsigned)h->num_shards, kBlockThreads, smem, st>>>(a);
         }
         if (mm.n_chains > 0) {
             TimedLaunch tl(h->timing, kClsFixup, st);
             k_fixup<R><<<(unsigned)mm.n_chains, 128, 0, st>>>(mm.chains, h->carry, out);
         }
-    } else if (fuse_from >= 0) {
-        h->cur = d;
-        h->remaps_done++;
     }
     MK_CUDA(cudaGetLastError());
     return MTTKRP_OK;
 }
 
 template <int N>
-static mttkrp_status_t launch_n(mttkrp_handle_s* h, int d, const float* const* factors, int R, float* out, int fuse_from,
-                                cudaStream_t st) {
+static mttkrp_status_t launch_n(mttkrp_handle_s* h, int d, const float* const* factors, int R, float* out, cudaStream_t st) {
     switch (R) {
-        case 8: return launch_nr<N, 8>(h, d, factors, out, fuse_from, st);
-        case 16: return launch_nr<N, 16>(h, d, factors, out, fuse_from, st);
-        case 32: return launch_nr<N, 32>(h, d, factors, out, fuse_from, st);
-        case 64: return launch_nr<N, 64>(h, d, factors, out, fuse_from, st);
+        case 8: return launch_nr<N, 8>(h, d, factors, out, st);
+        case 16: return launch_nr<N, 16>(h, d, factors, out, st);
+        case 32: return launch_nr<N, 32>(h, d, factors, out, st);
+        case 64: return launch_nr<N, 64>(h, d, factors, out, st);
     }
     set_error("unsupported rank %d (8, 16, 32, 64)", R);
     return MTTKRP_EUNSUPPORTED;
 }
 
-// fuse_from < 0: the resident copy is already in layout d.  fuse_from >= 0: it is in layout
-// fuse_from with (fuse_from + 1) % N == d, and the remap is done inside the MTTKRP kernel.
-mttkrp_status_t launch_mttkrp(mttkrp_handle_s* h, int d, const float* const* factors, int R, float* out, int fuse_from,
-                              cudaStream_t st) {
+// The resident copy must already be in layout d (api.cu runs the remap passes first).
+mttkrp_status_t launch_mttkrp(mttkrp_handle_s* h, int d, const float* const* factors, int R, float* out, cudaStream_t st) {
     switch (h->N) {
-        case 2: return launch_n<2>(h, d, factors, R, out, fuse_from, st);
-        case 3: return launch_n<3>(h, d, factors, R, out, fuse_from, st);
-        case 4: return launch_n<4>(h, d, factors, R, out, fuse_from, st);
-        case 5: return launch_n<5>(h, d, factors, R, out, fuse_from, st);
-        case 6: return launch_n<6>(h, d, factors, R, out, fuse_from, st);
-        case 7: return launch_n<7>(h, d, factors, R, out, fuse_from, st);
-        case 8: return launch_n<8>(h, d, factors, R, out, fuse_from, st);
+        case 2: return launch_n<2>(h, d, factors, R, out, st);
+        case 3: return launch_n<3>(h, d, factors, R, out, st);
+        case 4: return launch_n<4>(h, d, factors, R, out, st);
+        case 5: return launch_n<5>(h, d, factors, R, out, st);
+        case 6: return launch_n<6>(h, d, factors, R, out, st);
+        case 7: return launch_n<7>(h, d, factors, R, out, st);
+        case 8: return launch_n<8>(h, d, factors, R, out, st);
     }
     set_error("unsupported nmodes %d", h->N);
     return MTTKRP_EUNSUPPORTED;

@@ -5,40 +5,64 @@
 // the 16-byte loads.  On B200 the scatter form measured 2.3x slower (partial-sector writes turn
 // into read-modify-write in DRAM; profiles/r1_v1_ncu_summary.md).
 // Records are role-ordered (sort keys major to minor, then the value), so the pass also permutes
-// the index fields from the source layout's key order to the destination's, and it refreshes the
-// zero-valued padding records that fill the last shard.
+// the index fields from the source layout's key order to the destination's, refreshes the
+// zero-valued padding records that fill the last shard, and writes the destination layout's
+// run-end flags into bit 31 of the key words (common.cuh), which saves the MTTKRP kernel every
+// look-ahead compare.
 #include "common.cuh"
 
 namespace mk {
 
 struct FieldMap { int src[kMaxModes]; };   // out.field[l] = in.field[src[l]]
 
-// 3-mode records are 16 B: one 128-bit load and one 128-bit store per nonzero.
+// 3-mode records are 16 B: one 128-bit load and one 128-bit store per nonzero.  The run-end flags of
+// the destination layout (common.cuh) need the keys of destination record j+1: they come from the
+// next lane by shuffle; the last lane of a warp gathers that record itself.
 __global__ void __launch_bounds__(256) k_remap3(const uint4* __restrict__ in, const uint32_t* __restrict__ prev,
                                                 uint4* __restrict__ out, int64_t nnz, int64_t nnz_pad, FieldMap fm) {
-    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= nnz_pad) return;
-    const uint32_t src = __ldcs(prev + (j < nnz ? j : nnz - 1));
-    const uint4 r = __ldg(in + src);
-    const uint32_t f[3] = {r.x, r.y, r.z};
-    uint4 o;
-    o.x = fm.src[0] == 0 ? f[0] : (fm.src[0] == 1 ? f[1] : f[2]);
-    o.y = fm.src[1] == 0 ? f[0] : (fm.src[1] == 1 ? f[1] : f[2]);
-    o.z = fm.src[2] == 0 ? f[0] : (fm.src[2] == 1 ? f[1] : f[2]);
-    o.w = j < nnz ? r.w : 0u;
-    __stcs(out + j, o);
+    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;     // nnz_pad is a multiple of the block size
+    const int lane = threadIdx.x & 31;
+    auto gather = [&](int64_t jj, uint32_t* k, uint32_t& val) {
+        const uint32_t src = __ldcs(prev + (jj < nnz ? jj : nnz - 1));
+        const uint4 r = __ldg(in + src);
+        const uint32_t f[3] = {r.x & kKeyMask, r.y & kKeyMask, r.z & kKeyMask};
+#pragma unroll
+        for (int l = 0; l < 3; ++l) k[l] = fm.src[l] == 0 ? f[0] : (fm.src[l] == 1 ? f[1] : f[2]);
+        val = jj < nnz ? r.w : 0u;
+    };
+    uint32_t k[3], nk[3], val, nval;
+    gather(j, k, val);
+#pragma unroll
+    for (int l = 0; l < 3; ++l) nk[l] = __shfl_down_sync(0xffffffffu, k[l], 1);
+    const bool last = j + 1 >= nnz_pad;
+    if (lane == 31 && !last) gather(j + 1, nk, nval);
+    set_run_flags<3>(k, nk, last);
+    __stcs(out + j, make_uint4(k[0], k[1], k[2], val));
 }
 
 template <int N>
 __global__ void __launch_bounds__(256) k_remap(const uint32_t* __restrict__ in, const uint32_t* __restrict__ prev,
                                                uint32_t* __restrict__ out, int64_t nnz, int64_t nnz_pad, FieldMap fm) {
     const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= nnz_pad) return;
-    const uint32_t* r = in + (size_t)__ldcs(prev + (j < nnz ? j : nnz - 1)) * (N + 1);
+    const int lane = threadIdx.x & 31;
+    auto gather = [&](int64_t jj, uint32_t* k) {
+        const uint32_t* r = in + (size_t)__ldcs(prev + (jj < nnz ? jj : nnz - 1)) * (N + 1);
+#pragma unroll
+        for (int l = 0; l < N; ++l) k[l] = __ldg(r + fm.src[l]) & kKeyMask;
+        return r;
+    };
+    uint32_t k[N], nk[N];
+    const uint32_t* r = gather(j, k);
+    const uint32_t val = j < nnz ? __ldg(r + N) : 0u;
+#pragma unroll
+    for (int l = 0; l < N; ++l) nk[l] = __shfl_down_sync(0xffffffffu, k[l], 1);
+    const bool last = j + 1 >= nnz_pad;
+    if (lane == 31 && !last) gather(j + 1, nk);
+    set_run_flags<N>(k, nk, last);
     uint32_t* o = out + (size_t)j * (N + 1);
 #pragma unroll
-    for (int l = 0; l < N; ++l) o[l] = __ldg(r + fm.src[l]);
-    o[N] = j < nnz ? __ldg(r + N) : 0u;
+    for (int l = 0; l < N; ++l) o[l] = k[l];
+    o[N] = val;
 }
 
 mttkrp_status_t launch_remap(mttkrp_handle_s* h, int from, cudaStream_t st) {
@@ -94,7 +118,7 @@ __global__ void k_export(const uint32_t* __restrict__ rec, int64_t nnz, int N, P
     int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= nnz) return;
     const uint32_t* r = rec + (size_t)k * (N + 1);
-    for (int m = 0; m < N; ++m) idx[(size_t)m * nnz + k] = (int32_t)r[pos.v[m]];
+    for (int m = 0; m < N; ++m) idx[(size_t)m * nnz + k] = (int32_t)(r[pos.v[m]] & kKeyMask);
     vals[k] = __uint_as_float(r[N]);
 }
 

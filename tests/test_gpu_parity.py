@@ -190,18 +190,6 @@ def test_errors_are_reported(P):
     h.destroy()
 
 
-def test_fused_remap_variant(P, monkeypatch):
-    # MTTKRP_FUSE=1: the last remap step runs inside the MTTKRP kernel (the paper's Alg. 4 layout of
-    # work).  Same contract: remapped copy bit-exact, Y within tolerance, any call order.
-    monkeypatch.setenv("MTTKRP_FUSE", "1")
-    for cfg, nnz, R in [(0, 40_013, 16), (1, 150_001, 32), (3, 90_007, 32), (4, 90_007, 8)]:
-        spec = W.CONFIGS[cfg].scaled(nnz)
-        t = W.generate_tensor(spec)
-        N = len(spec.dims)
-        order = list(range(N)) + [0, 1] + [N - 1, 1]
-        _run_case(P, spec.dims, t.idx, t.vals, R, seed=6, order_modes=order)
-
-
 def _sample_rows(idx_d, dim, rng, k=48):
     """Heaviest rows, rows around shard boundaries' worth of mass, and random rows."""
     counts = torch.bincount(idx_d.long(), minlength=dim)
