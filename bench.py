@@ -33,7 +33,7 @@ FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallba
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (0-based)")
     ap.add_argument("--rank", type=int, default=0, help="R (0 = the config's)")
@@ -314,6 +314,8 @@ def run_ours(args):
                            "checksums": checksums, "distinct_per_mode": U, "shard_nnz": info["shard_nnz"],
                            "num_shards": info["num_shards"], "split_rows": info["num_split_rows"],
                            "empty_rows": info["num_empty_rows"], "key_order": info["key_order"],
+                           "remap_blocked": info["remap_blocked"],
+                           "remap_avg_run": [round(x, 1) for x in info["remap_avg_run"]],
                            "bytes_held": info["bytes_held"], "bytes_paper_format": info["bytes_paper_format"],
                            "create_s": t_create, "generate_s": t_gen},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_sweep * args.steps,

@@ -67,6 +67,11 @@ typedef struct {
     int32_t key_order[MTTKRP_MAX_MODES][MTTKRP_MAX_MODES];
                                          /* key_order[d] = sort-key order of the mode-d layout:
                                             key_order[d][0] == d, then the other modes (major to minor) */
+    int32_t remap_blocked[MTTKRP_MAX_MODES];
+                                         /* 1: the remap d -> (d+1)%N walks the destination in source-block order
+                                            (L2-resident gather window), 0: in destination order */
+    double remap_avg_run[MTTKRP_MAX_MODES];
+                                         /* average length of the ascending destination runs of that walk */
 } mttkrp_info_t;
 
 /*
@@ -101,7 +106,7 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
  *   out:     device fp32 [dims[d]][R] row-major; fully overwritten (rows without nonzeros get 0).
  *            Must not alias a factor that is read.
  *   Any d in any order.  If the resident layout is not d the tensor is first remapped
- *   (cur -> cur+1 -> ... -> d, one scatter pass per step; the cyclic order of Alg. 5 costs one).
+ *   (cur -> cur+1 -> ... -> d, one gather pass per step; the cyclic order of Alg. 5 costs one).
  */
 mttkrp_status_t mttkrp_mode(mttkrp_handle_t h, int d, const float* const* factors, int R,
                             float* out, void* cuda_stream);

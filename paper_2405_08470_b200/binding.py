@@ -37,7 +37,8 @@ class Info(ctypes.Structure):
                 ("shard_nnz", ctypes.c_int32), ("num_shards", ctypes.c_int64),
                 ("num_split_rows", ctypes.c_int64 * MAX_MODES), ("num_empty_rows", ctypes.c_int64 * MAX_MODES),
                 ("bytes_held", ctypes.c_int64), ("bytes_paper_format", ctypes.c_int64),
-                ("remaps_done", ctypes.c_int64), ("key_order", (ctypes.c_int32 * MAX_MODES) * MAX_MODES)]
+                ("remaps_done", ctypes.c_int64), ("key_order", (ctypes.c_int32 * MAX_MODES) * MAX_MODES),
+                ("remap_blocked", ctypes.c_int32 * MAX_MODES), ("remap_avg_run", ctypes.c_double * MAX_MODES)]
 
 
 class Timing(ctypes.Structure):
@@ -213,6 +214,7 @@ class Mttkrp:
             "bytes_held": raw.bytes_held, "bytes_paper_format": raw.bytes_paper_format,
             "remaps_done": raw.remaps_done,
             "key_order": [list(raw.key_order[d])[:n] for d in range(n)],
+            "remap_blocked": list(raw.remap_blocked)[:n], "remap_avg_run": list(raw.remap_avg_run)[:n],
         }
 
     def get_perm(self, d: int) -> torch.Tensor:

@@ -19,7 +19,7 @@ void set_error(const char* fmt, ...) {
     va_end(ap);
 }
 
-void choose_key_order(int N, const int64_t* dims, int d, int* order);   // build.cu
+void choose_key_order(int N, const int64_t* dims, int d, const char* env, int* order);   // build.cu
 
 static mttkrp_status_t check_shape(int nmodes, const int64_t* dims, int64_t nnz) {
     if (!dims) { set_error("dims is NULL"); return MTTKRP_EINVAL; }
@@ -111,11 +111,25 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
     h->max_rank = max_rank;
     h->device = dev;
     h->timing = new (std::nothrow) Timing();
+    // Key order of the layouts (reading 4).  The default makes every remap a stable partition
+    // by one key, which the blocked remap turns into L2-resident gathers; that pays when the nonzeros a
+    // source block sends to one output row form runs of several records.  The expected run for mode d
+    // is nnz / (dims[d] * number of blocks); when most modes are too large for that, the size-ordered
+    // tuple (one remap of the cycle moves whole fibers) is the better choice.
+    const char* order_env = getenv("MTTKRP_KEY_ORDER");
+    if (!order_env) {
+        const double nblk = (double)((nnz >> 20) > 0 ? (nnz >> 20) : 1);
+        int good = 0;
+        for (int d = 0; d < nmodes; ++d) good += ((double)nnz / ((double)dims[d] * nblk) >= 1.0) ? 1 : 0;
+        order_env = (2 * good >= nmodes) ? "revcyclic" : "desc";
+    }
     for (int d = 0; d < nmodes; ++d) {
         ModeMeta& mm = h->mode[d];
-        choose_key_order(nmodes, dims, d, mm.order);
+        choose_key_order(nmodes, dims, d, order_env, mm.order);
         for (int l = 0; l < nmodes; ++l) mm.pos[mm.order[l]] = l;
         mm.next = reinterpret_cast<uint32_t*>(ws + p.next[d]);
+        mm.ord = reinterpret_cast<uint32_t*>(ws + p.ord[d]);
+        mm.lflags = reinterpret_cast<uint8_t*>(ws + p.lflags[d]);
         mm.empty_rows = reinterpret_cast<uint32_t*>(ws + p.empty[d]);
         mm.chains = reinterpret_cast<uint32_t*>(ws + p.chains[d]);
         if (max_rank > 0) {
@@ -239,6 +253,8 @@ mttkrp_status_t mttkrp_get_info(mttkrp_handle_t h, mttkrp_info_t* info) {
         info->num_split_rows[m] = h->mode[m].n_chains;
         info->num_empty_rows[m] = h->mode[m].n_empty;
         for (int l = 0; l < h->N; ++l) info->key_order[m][l] = h->mode[m].order[l];
+        info->remap_blocked[m] = h->mode[m].blocked;
+        info->remap_avg_run[m] = h->mode[m].avg_run;
         bits += ceil_log2(h->dims[m]);
     }
     bits += (int64_t)h->N * ceil_log2(h->nnz > 1 ? h->nnz : 2);

@@ -40,6 +40,8 @@ mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_
     size_t off = 0;
     p->rec_a = off; off = align_up(off + rec_bytes);
     for (int d = 0; d < N; ++d) { p->next[d] = off; off = align_up(off + 4 * n); }
+    for (int d = 0; d < N; ++d) { p->ord[d] = off; off = align_up(off + 4 * n); }
+    for (int d = 0; d < N; ++d) { p->lflags[d] = off; off = align_up(off + (size_t)(p->num_shards * p->shard_nnz)); }
     p->perm0 = off; off = align_up(off + 4 * n);
     for (int d = 0; d < N; ++d) { p->empty[d] = off; off = align_up(off + 4 * (size_t)dims[d]); }
     for (int d = 0; d < N; ++d) { p->chains[d] = off; off = align_up(off + 12 * (size_t)p->num_shards); }
@@ -268,30 +270,58 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_scatter(const uint32_t* 
 // rec[k] = { idx[order[0]][perm[k]], ..., idx[order[N-1]][perm[k]], val[perm[k]] }
 struct OrderArg { int v[kMaxModes]; };
 
-// Positions k in [nnz, nnz_pad) are padding: the keys of the last nonzero with value 0.  Bit 31 of
-// the key words gets the run-end flags (common.cuh), from the keys of the record at k+1.
+// Run-end flags of one layout (common.cuh): bit l of flags[k] = e_l = "the record at k+1 differs from
+// the record at k in one of the keys k_0..k_l".  Padding positions repeat the last nonzero (no run
+// ends); the last position of the padded array has every flag set.
+__global__ void k_build_flags(const int32_t* __restrict__ idx, const uint32_t* __restrict__ perm, int64_t nnz,
+                              int64_t nnz_pad, int N, OrderArg order, uint8_t* __restrict__ flags) {
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nnz_pad) return;
+    const bool last = k + 1 >= nnz_pad;
+    const uint32_t src = perm[k < nnz ? k : nnz - 1];
+    const uint32_t nsrc = last ? src : perm[k + 1 < nnz ? k + 1 : nnz - 1];
+    bool diff = last;
+    uint32_t f = 0;
+    for (int l = 0; l < N - 1; ++l) {
+        const size_t col = (size_t)order.v[l] * nnz;
+        diff = diff || (idx[col + src] != idx[col + nsrc]);
+        f |= (diff ? 1u : 0u) << l;
+    }
+    flags[k] = (uint8_t)f;
+}
+
+// rec[k] = keys of the nonzero perm[k] in the layout's key order (with its run-end flags merged into
+// bit 31, common.cuh) + value.  Positions k in [nnz, nnz_pad) are padding: the keys of the last
+// nonzero with value 0.
 __global__ void k_build_records(const int32_t* __restrict__ idx, const float* __restrict__ vals,
-                                const uint32_t* __restrict__ perm, int64_t nnz, int64_t nnz_pad, int N, OrderArg order,
-                                uint32_t* __restrict__ rec) {
+                                const uint32_t* __restrict__ perm, const uint8_t* __restrict__ flags, int64_t nnz,
+                                int64_t nnz_pad, int N, OrderArg order, uint32_t* __restrict__ rec) {
     int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= nnz_pad) return;
     const uint32_t src = perm[k < nnz ? k : nnz - 1];
-    const bool last = k + 1 >= nnz_pad;
-    const uint32_t nsrc = last ? src : perm[k + 1 < nnz ? k + 1 : nnz - 1];
+    const uint32_t f = flags[k];
     uint32_t* r = rec + (size_t)k * (N + 1);
-    bool diff = last, e0 = false;
     for (int l = 0; l < N; ++l) {
-        const uint32_t key = (uint32_t)idx[(size_t)order.v[l] * nnz + src];
-        uint32_t flag = 0u;
-        if (l < N - 1) {
-            diff = diff || ((uint32_t)idx[(size_t)order.v[l] * nnz + nsrc] != key);
-            if (l == 0) e0 = diff;
-            else flag = diff ? kFlag : 0u;
-        }
-        if (l == N - 1) flag = e0 ? kFlag : 0u;
-        r[l] = key | (l == 0 ? 0u : flag);
+        uint32_t key = (uint32_t)idx[(size_t)order.v[l] * nnz + src];
+        if (l >= 1 && l <= N - 2) key |= ((f >> l) & 1u) << 31;
+        if (l == N - 1) key |= (f & 1u) << 31;
+        r[l] = key;
     }
     r[N] = k < nnz ? __float_as_uint(vals[src]) : 0u;
+}
+
+// key[j] = map[j] >> shift (the source block of destination position j)
+__global__ void k_block_keys(const uint32_t* __restrict__ map, int shift, uint32_t* __restrict__ key, int64_t n) {
+    int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j < n) key[j] = map[j] >> shift;
+}
+
+// counts the positions t with ord[t+1] != ord[t] + 1 (run breaks)
+__global__ void k_count_breaks(const uint32_t* __restrict__ ord, int64_t n, uint32_t* __restrict__ counter) {
+    int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool brk = (t + 1 < n) && (ord[t + 1] != ord[t] + 1u);
+    const unsigned m = __ballot_sync(0xffffffffu, brk);
+    if ((threadIdx.x & 31) == 0 && m) atomicAdd(counter, (uint32_t)__popc(m));
 }
 
 __global__ void k_mark_rows(const uint32_t* __restrict__ kd, int64_t nnz, uint32_t* __restrict__ present) {
@@ -355,21 +385,28 @@ static int ceil_log2_i64(int64_t x) {
     return b;
 }
 
-void choose_key_order(int N, const int64_t* dims, int d, int* order) {
-    // order[0] = d; the other modes by descending size (ties: lower mode first), so the largest
-    // input factor is the one reused along a fiber and the smallest, most cacheable one is the
-    // per-nonzero gather (reading 4).  MTTKRP_KEY_ORDER=asc|cyclic overrides (tuning).
-    const char* env = getenv("MTTKRP_KEY_ORDER");
+void choose_key_order(int N, const int64_t* dims, int d, const char* env, int* order) {
+    // Default: order[d] = (d, d-1, d-2, ..., d-N+1) (mod N).  The layout of mode d+1 is then
+    // (last key of layout d, then the keys of layout d in their order), so inside one output row of
+    // mode d+1 the nonzeros appear in the same order as in layout d: the remap d -> d+1 is a stable
+    // partition by a single key, and the nonzeros that a block of layout d sends to one output row
+    // stay contiguous (what the blocked remap needs, remap.cu).  DESIGN.md reading 4.
+    // `env` (mttkrp_create: MTTKRP_KEY_ORDER, or "desc" when the modes are too large for the blocked
+    // remap to pay) selects other tuples: desc / asc = the other modes by size, cyclic = d+1, d+2, ...
+    order[0] = d;
+    if (!env || strcmp(env, "revcyclic") == 0) {
+        for (int j = 1; j < N; ++j) order[j] = ((d - j) % N + N) % N;
+        return;
+    }
     int rest[kMaxModes], n = 0;
     for (int j = 1; j < N; ++j) rest[n++] = (d + j) % N;     // cyclic
-    if (!env || strcmp(env, "cyclic") != 0) {
-        bool asc = env && strcmp(env, "asc") == 0;
+    if (strcmp(env, "cyclic") != 0) {
+        bool asc = strcmp(env, "asc") == 0;
         std::sort(rest, rest + n, [&](int a, int b) {
             if (dims[a] != dims[b]) return asc ? dims[a] < dims[b] : dims[a] > dims[b];
             return a < b;
         });
     }
-    order[0] = d;
     for (int j = 0; j < n; ++j) order[j + 1] = rest[j];
 }
 
@@ -437,6 +474,12 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
                 MK_CUDA(cudaGetLastError());
             }
             // pa = perm_d, ka = idx[d] in mode-d order
+            {
+                OrderArg oa;
+                for (int l = 0; l < kMaxModes; ++l) oa.v[l] = mm.order[l];
+                const int64_t nnz_pad = nshards * (int64_t)S;
+                k_build_flags<<<grid_for(nnz_pad, 256), 256, 0, st>>>(idx, pa, nnz, nnz_pad, N, oa, mm.lflags);
+            }
             MK_CUDA(cudaMemcpyAsync(dst, pa, 4 * n, cudaMemcpyDeviceToDevice, st));
             if (d == 0) MK_CUDA(cudaMemcpyAsync(h->perm0, pa, 4 * n, cudaMemcpyDeviceToDevice, st));
 
@@ -469,7 +512,7 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
         OrderArg oa;
         for (int l = 0; l < kMaxModes; ++l) oa.v[l] = h->mode[0].order[l];
         const int64_t nnz_pad = nshards * (int64_t)S;
-        k_build_records<<<grid_for(nnz_pad, 256), 256, 0, st>>>(idx, vals, h->perm0, nnz, nnz_pad, N, oa, h->rec_cur);
+        k_build_records<<<grid_for(nnz_pad, 256), 256, 0, st>>>(idx, vals, h->perm0, h->mode[0].lflags, nnz, nnz_pad, N, oa, h->rec_cur);
         // Slot d still holds perm_d; go d = 0..N-1, the last one needs perm_0, which slot 0 no longer
         // holds -> use the perm0 copy.
         uint32_t* inv = keyA;
@@ -481,14 +524,50 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
             k_gather_u32<<<grid_for(nnz, 256), 256, 0, st>>>(inv, perm_e, h->mode[d].next, nnz);
         }
         MK_CUDA(cudaGetLastError());
+        // Blocked remap order (remap.cu): destination positions of the remap d -> d+1 grouped, stably,
+        // by the source block they read from: one 8-bit radix pass on the block id.  The block is sized
+        // to stay L2-resident while the whole grid gathers from it.
+        int block_log2 = 20;
+        {
+            const char* env = getenv("MTTKRP_REMAP_BLOCK_LOG2");
+            if (env) block_log2 = atoi(env);
+            if (block_log2 < 10) block_log2 = 10;
+            while ((nnz >> block_log2) > 255) ++block_log2;            // at most 256 blocks (one radix digit)
+        }
+        for (int d = 0; d < N; ++d) {
+            ModeMeta& mm = h->mode[d];
+            mm.block_log2 = block_log2;
+            k_block_keys<<<grid_for(nnz, 256), 256, 0, st>>>(mm.next, block_log2, keyA, nnz);
+            k_iota<<<grid_for(nnz, 256), 256, 0, st>>>(permA, nnz);
+            k_radix_hist<<<(unsigned)nblocks, kSortThreads, 0, st>>>(keyA, nnz, 0, hist, nblocks);
+            MK_TRY(exclusive_scan(hist, 256 * nblocks, sums, st));
+            k_radix_scatter<<<(unsigned)nblocks, kSortThreads, 0, st>>>(keyA, permA, keyB, mm.ord, nnz, 0, hist, nblocks);
+            k_count_breaks<<<grid_for(nnz, 256), 256, 0, st>>>(mm.ord, nnz, small + 32 + d);
+            k_count_breaks<<<grid_for(nnz, 256), 256, 0, st>>>(mm.next, nnz, small + 40 + d);
+        }
+        MK_CUDA(cudaGetLastError());
     }
 
-    uint32_t counts[2 * kMaxModes] = {0};
+    uint32_t counts[2 * kMaxModes] = {0}, breaks[2 * kMaxModes] = {0};
     MK_CUDA(cudaMemcpyAsync(counts, small + 8, sizeof(uint32_t) * 2 * N, cudaMemcpyDeviceToHost, st));
+    MK_CUDA(cudaMemcpyAsync(breaks, small + 32, sizeof(uint32_t) * 2 * kMaxModes, cudaMemcpyDeviceToHost, st));
     MK_CUDA(cudaStreamSynchronize(st));
+    const char* benv = getenv("MTTKRP_REMAP_BLOCKED");           // 0 / 1 force the choice (experiments)
     for (int d = 0; d < N; ++d) {
         h->mode[d].n_chains = nnz > 0 ? counts[2 * d] : 0;
         h->mode[d].n_empty = nnz > 0 ? counts[2 * d + 1] : h->dims[d];
+        // Use the blocked order when the source window fits L2 comfortably, the destination runs are
+        // long enough to store whole sectors (average run >= 4 records), and the plain walk is a random
+        // gather (when consecutive destinations read consecutive sources - a remap that moves whole
+        // fibers - the plain walk is already sequential on both sides).
+        const int64_t runs = (int64_t)breaks[d] + 1;
+        const int64_t src_runs = (int64_t)breaks[kMaxModes + d] + 1;
+        const bool fits = ((int64_t)(N + 1) * 4 << h->mode[d].block_log2) <= (48ll << 20);
+        bool blocked = nnz > 0 && fits && (nnz >> h->mode[d].block_log2) >= 2 && nnz / runs >= 4 &&
+                       (double)nnz / (double)src_runs < 1.5;
+        if (benv) blocked = nnz > 0 && benv[0] == '1';
+        h->mode[d].blocked = blocked ? 1 : 0;
+        h->mode[d].avg_run = nnz > 0 ? (double)nnz / (double)runs : 0.0;
     }
     return MTTKRP_OK;
 }

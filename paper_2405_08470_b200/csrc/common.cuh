@@ -40,18 +40,13 @@ void set_error(const char* fmt, ...);
 constexpr uint32_t kFlag = 0x80000000u;
 constexpr uint32_t kKeyMask = 0x7fffffffu;
 
-// flags of a record from its keys `k` and the keys `nk` of the record after it (sorted order)
+// The flags are a property of (layout, position), so mttkrp_create computes them once per layout into a
+// byte array (bit l = e_l) and the record builder / remap pass only merges them into the key words.
 template <int N>
-__device__ __forceinline__ void set_run_flags(uint32_t* k, const uint32_t* nk, bool last_of_array) {
-    bool diff = last_of_array;
-    bool e0 = false;
+__device__ __forceinline__ void apply_run_flags(uint32_t* k, uint32_t f) {
 #pragma unroll
-    for (int l = 0; l < N - 1; ++l) {
-        diff = diff || (nk[l] != k[l]);
-        if (l == 0) e0 = diff;
-        else k[l] |= diff ? kFlag : 0u;
-    }
-    k[N - 1] |= e0 ? kFlag : 0u;
+    for (int l = 1; l < N - 1; ++l) k[l] |= ((f >> l) & 1u) << 31;
+    k[N - 1] |= (f & 1u) << 31;
 }
 
 // Per-mode tables built by mttkrp_create.
@@ -60,6 +55,13 @@ struct ModeMeta {
     int pos[kMaxModes];       // pos[m] = level of mode m in `order`
     uint32_t* next;           // [nnz] gather map of the remap d -> (d+1)%N: position in THIS layout of the
                               // element at position j of the next layout (the paper's remap id, read backwards)
+    uint32_t* ord;            // [nnz] positions of the NEXT layout ordered by the 2^block_log2-record block of this
+                              // layout they come from (stable), or unused: the blocked remap walks the destination
+                              // in this order so that its random reads stay inside one L2-resident window at a time
+    int blocked;              // 1: the remap d -> (d+1)%N uses `ord`
+    int block_log2;
+    double avg_run;           // average length of the ascending destination runs in `ord`
+    uint8_t* lflags;          // [nnz_pad] run-end flags of THIS layout: bit l = e_l (see "Run-end flags")
     uint32_t* empty_rows;     // [n_empty] output rows without a nonzero
     int64_t n_empty;
     uint32_t* chains;         // [n_chains][3] = {first shard, last shard, row} for rows spanning shards
@@ -120,7 +122,7 @@ namespace mk {
 // ---- build.cu -------------------------------------------------------------------------------
 struct WorkspacePlan {
     size_t rec_a, rec_b, perm0, carry;
-    size_t next[kMaxModes], empty[kMaxModes], chains[kMaxModes];
+    size_t next[kMaxModes], empty[kMaxModes], chains[kMaxModes], ord[kMaxModes], lflags[kMaxModes];
     size_t stage_fac[kMaxModes], stage_out[kMaxModes];
     size_t persistent_end;
     size_t scratch;          // start of the create-time scratch (may overlap rec_b)

@@ -6,63 +6,67 @@
 // into read-modify-write in DRAM; profiles/r1_v1_ncu_summary.md).
 // Records are role-ordered (sort keys major to minor, then the value), so the pass also permutes
 // the index fields from the source layout's key order to the destination's, refreshes the
-// zero-valued padding records that fill the last shard, and writes the destination layout's
-// run-end flags into bit 31 of the key words (common.cuh), which saves the MTTKRP kernel every
-// look-ahead compare.
+// zero-valued padding records that fill the last shard, and merges the destination layout's
+// precomputed run-end flags into bit 31 of the key words (common.cuh), which saves the MTTKRP
+// kernel every look-ahead compare.
 #include "common.cuh"
 
 namespace mk {
 
 struct FieldMap { int src[kMaxModes]; };   // out.field[l] = in.field[src[l]]
 
-// 3-mode records are 16 B: one 128-bit load and one 128-bit store per nonzero.  The run-end flags of
-// the destination layout (common.cuh) need the keys of destination record j+1: they come from the
-// next lane by shuffle; the last lane of a warp gathers that record itself.
+// 3-mode records are 16 B: one 128-bit load and one 128-bit store per nonzero.
+// BLOCKED: thread t handles destination position ord[t] instead of t.  `ord` lists the destination
+// positions grouped by the source block (2^block_log2 records) their record comes from, so at any
+// time the whole grid gathers from one source window that stays in L2, and every 64-byte DRAM
+// fetch is used completely; inside a group the destination positions ascend in long runs (the
+// layouts' key orders are chosen for that, build.cu choose_key_order), so the stores stay whole sectors.
+template <bool BLOCKED>
 __global__ void __launch_bounds__(256) k_remap3(const uint4* __restrict__ in, const uint32_t* __restrict__ prev,
+                                                const uint32_t* __restrict__ ord, const uint8_t* __restrict__ dflags,
                                                 uint4* __restrict__ out, int64_t nnz, int64_t nnz_pad, FieldMap fm) {
-    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;     // nnz_pad is a multiple of the block size
-    const int lane = threadIdx.x & 31;
-    auto gather = [&](int64_t jj, uint32_t* k, uint32_t& val) {
-        const uint32_t src = __ldcs(prev + (jj < nnz ? jj : nnz - 1));
-        const uint4 r = __ldg(in + src);
-        const uint32_t f[3] = {r.x & kKeyMask, r.y & kKeyMask, r.z & kKeyMask};
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= nnz_pad) return;
+    const int64_t j = (BLOCKED && t < nnz) ? (int64_t)__ldcs(ord + t) : t;   // padding positions are handled in place
+    const uint32_t src = BLOCKED ? __ldg(prev + (j < nnz ? j : nnz - 1)) : __ldcs(prev + (j < nnz ? j : nnz - 1));
+    const uint4 r = __ldg(in + src);
+    const uint32_t f[3] = {r.x & kKeyMask, r.y & kKeyMask, r.z & kKeyMask};
+    uint32_t k[3];
 #pragma unroll
-        for (int l = 0; l < 3; ++l) k[l] = fm.src[l] == 0 ? f[0] : (fm.src[l] == 1 ? f[1] : f[2]);
-        val = jj < nnz ? r.w : 0u;
-    };
-    uint32_t k[3], nk[3], val, nval;
-    gather(j, k, val);
-#pragma unroll
-    for (int l = 0; l < 3; ++l) nk[l] = __shfl_down_sync(0xffffffffu, k[l], 1);
-    const bool last = j + 1 >= nnz_pad;
-    if (lane == 31 && !last) gather(j + 1, nk, nval);
-    set_run_flags<3>(k, nk, last);
-    __stcs(out + j, make_uint4(k[0], k[1], k[2], val));
+    for (int l = 0; l < 3; ++l) k[l] = fm.src[l] == 0 ? f[0] : (fm.src[l] == 1 ? f[1] : f[2]);
+    apply_run_flags<3>(k, dflags[j]);
+    __stcs(out + j, make_uint4(k[0], k[1], k[2], j < nnz ? r.w : 0u));
 }
 
-template <int N>
+template <int N, bool BLOCKED>
 __global__ void __launch_bounds__(256) k_remap(const uint32_t* __restrict__ in, const uint32_t* __restrict__ prev,
+                                               const uint32_t* __restrict__ ord, const uint8_t* __restrict__ dflags,
                                                uint32_t* __restrict__ out, int64_t nnz, int64_t nnz_pad, FieldMap fm) {
-    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const int lane = threadIdx.x & 31;
-    auto gather = [&](int64_t jj, uint32_t* k) {
-        const uint32_t* r = in + (size_t)__ldcs(prev + (jj < nnz ? jj : nnz - 1)) * (N + 1);
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= nnz_pad) return;
+    const int64_t j = (BLOCKED && t < nnz) ? (int64_t)__ldcs(ord + t) : t;
+    const uint32_t* r = in + (size_t)__ldg(prev + (j < nnz ? j : nnz - 1)) * (N + 1);
+    uint32_t k[N];
 #pragma unroll
-        for (int l = 0; l < N; ++l) k[l] = __ldg(r + fm.src[l]) & kKeyMask;
-        return r;
-    };
-    uint32_t k[N], nk[N];
-    const uint32_t* r = gather(j, k);
-    const uint32_t val = j < nnz ? __ldg(r + N) : 0u;
-#pragma unroll
-    for (int l = 0; l < N; ++l) nk[l] = __shfl_down_sync(0xffffffffu, k[l], 1);
-    const bool last = j + 1 >= nnz_pad;
-    if (lane == 31 && !last) gather(j + 1, nk);
-    set_run_flags<N>(k, nk, last);
+    for (int l = 0; l < N; ++l) k[l] = __ldg(r + fm.src[l]) & kKeyMask;
+    apply_run_flags<N>(k, dflags[j]);
     uint32_t* o = out + (size_t)j * (N + 1);
 #pragma unroll
     for (int l = 0; l < N; ++l) o[l] = k[l];
-    o[N] = val;
+    o[N] = j < nnz ? __ldg(r + N) : 0u;
+}
+
+template <int N>
+static void launch_remap_n(mttkrp_handle_s* h, int from, int to, unsigned grid, int64_t nnz_pad, const FieldMap& fm, cudaStream_t st) {
+    const ModeMeta& mf = h->mode[from];
+    const uint8_t* dflags = h->mode[to].lflags;
+    if constexpr (N == 3) {
+        if (mf.blocked) k_remap3<true><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, mf.next, mf.ord, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, fm);
+        else k_remap3<false><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, mf.next, mf.ord, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, fm);
+    } else {
+        if (mf.blocked) k_remap<N, true><<<grid, 256, 0, st>>>(h->rec_cur, mf.next, mf.ord, dflags, h->rec_alt, h->nnz, nnz_pad, fm);
+        else k_remap<N, false><<<grid, 256, 0, st>>>(h->rec_cur, mf.next, mf.ord, dflags, h->rec_alt, h->nnz, nnz_pad, fm);
+    }
 }
 
 mttkrp_status_t launch_remap(mttkrp_handle_s* h, int from, cudaStream_t st) {
@@ -74,16 +78,15 @@ mttkrp_status_t launch_remap(mttkrp_handle_s* h, int from, cudaStream_t st) {
         for (int l = 0; l < N; ++l) fm.src[l] = h->mode[from].pos[h->mode[to].order[l]];
         const int64_t nnz_pad = h->num_shards * (int64_t)h->shard_nnz;
         const unsigned grid = (unsigned)((nnz_pad + 255) / 256);
-        const uint32_t* prev = h->mode[from].next;
         TimedLaunch tl(h->timing, kClsRemap, st);
         switch (N) {
-            case 2: k_remap<2><<<grid, 256, 0, st>>>(h->rec_cur, prev, h->rec_alt, h->nnz, nnz_pad, fm); break;
-            case 3: k_remap3<<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, prev, (uint4*)h->rec_alt, h->nnz, nnz_pad, fm); break;
-            case 4: k_remap<4><<<grid, 256, 0, st>>>(h->rec_cur, prev, h->rec_alt, h->nnz, nnz_pad, fm); break;
-            case 5: k_remap<5><<<grid, 256, 0, st>>>(h->rec_cur, prev, h->rec_alt, h->nnz, nnz_pad, fm); break;
-            case 6: k_remap<6><<<grid, 256, 0, st>>>(h->rec_cur, prev, h->rec_alt, h->nnz, nnz_pad, fm); break;
-            case 7: k_remap<7><<<grid, 256, 0, st>>>(h->rec_cur, prev, h->rec_alt, h->nnz, nnz_pad, fm); break;
-            case 8: k_remap<8><<<grid, 256, 0, st>>>(h->rec_cur, prev, h->rec_alt, h->nnz, nnz_pad, fm); break;
+            case 2: launch_remap_n<2>(h, from, to, grid, nnz_pad, fm, st); break;
+            case 3: launch_remap_n<3>(h, from, to, grid, nnz_pad, fm, st); break;
+            case 4: launch_remap_n<4>(h, from, to, grid, nnz_pad, fm, st); break;
+            case 5: launch_remap_n<5>(h, from, to, grid, nnz_pad, fm, st); break;
+            case 6: launch_remap_n<6>(h, from, to, grid, nnz_pad, fm, st); break;
+            case 7: launch_remap_n<7>(h, from, to, grid, nnz_pad, fm, st); break;
+            case 8: launch_remap_n<8>(h, from, to, grid, nnz_pad, fm, st); break;
             default: set_error("remap: unsupported nmodes %d", N); return MTTKRP_EUNSUPPORTED;
         }
         MK_CUDA(cudaGetLastError());
