@@ -260,13 +260,13 @@ def run_ours(args):
         peak, peak_src = FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
     alg_bytes_launch = sum(bytes_mode) / N
     achieved = alg_bytes_launch / (k_ms * 1e-3) / 1e9 if k_ms > 0 else 0.0
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    traffic = None                                     # ncu dram bytes per launch of that kernel (profiles/r1_traffic.csv)
+    tpath = os.path.join(ROOT, "profiles", "r1_traffic.csv")
     if os.path.exists(tpath):
-        try:
-            traffic = json.load(open(tpath)).get(f"config{args.config}", {}).get("k_mttkrp_dram_bytes_per_launch")
-        except Exception:
-            traffic = None
+        import csv
+        for row in csv.DictReader(open(tpath)):
+            if row["config"] == str(args.config) and row["kernel"] == "k_mttkrp" and not args.nnz and not args.rank:
+                traffic = float(row["dram_bytes_per_launch"])
     total_k = tm["remap_ms"] + tm["zero_ms"] + tm["mttkrp_ms"] + tm["fixup_ms"]
     roofline = {"bound": "hbm", "kernel": "k_mttkrp", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,

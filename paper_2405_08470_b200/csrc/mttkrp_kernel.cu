@@ -127,7 +127,7 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 // ---- compile-time geometry ---------------------------------------------------------------------
 #ifndef MK_V8
 #define MK_V8 0          // 1: 8 columns per lane (256-bit gathers); measured 1.4 L1 wavefronts per 128-byte line
-#endif                   //    against 1.0 for 128-bit gathers (profiles/r1_probe_gather.md)
+#endif                   //    against 1.0 for 128-bit gathers
 #ifndef MK_D
 #define MK_D 2
 #endif
