@@ -44,7 +44,7 @@ typedef enum {
     MTTKRP_OK = 0,
     MTTKRP_EINVAL = 1,       /* bad argument (null pointer, size, mode, rank, alignment) */
     MTTKRP_EINDEX = 2,       /* an index is outside [0, dims[m]) (detected on the device in create) */
-    MTTKRP_EUNSUPPORTED = 3, /* nmodes outside [2,8], R not in {8,16,32,64}, nnz >= 2^31 */
+    MTTKRP_EUNSUPPORTED = 3, /* nmodes outside [2,8], R not in {8,16,32,64}, nnz >= 2^31, a dimension >= 2^28 */
     MTTKRP_EWORKSPACE = 4,   /* workspace too small or misaligned */
     MTTKRP_ECUDA = 5         /* a CUDA runtime call or kernel launch failed */
 } mttkrp_status_t;

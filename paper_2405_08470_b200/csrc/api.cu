@@ -26,7 +26,7 @@ static mttkrp_status_t check_shape(int nmodes, const int64_t* dims, int64_t nnz)
     if (nmodes < 2 || nmodes > kMaxModes) { set_error("nmodes %d outside [2,%d]", nmodes, kMaxModes); return MTTKRP_EUNSUPPORTED; }
     for (int m = 0; m < nmodes; ++m) {
         if (dims[m] <= 0) { set_error("dims[%d] = %lld must be positive", m, (long long)dims[m]); return MTTKRP_EINVAL; }
-        if (dims[m] > 0x7fffffffLL) { set_error("dims[%d] exceeds int32", m); return MTTKRP_EUNSUPPORTED; }
+        if (dims[m] >= (1LL << 28)) { set_error("dims[%d] >= 2^28 unsupported", m); return MTTKRP_EUNSUPPORTED; }
     }
     if (nnz < 0) { set_error("nnz < 0"); return MTTKRP_EINVAL; }
     if (nnz >= 0x7fffffffLL) { set_error("nnz >= 2^31 unsupported"); return MTTKRP_EUNSUPPORTED; }

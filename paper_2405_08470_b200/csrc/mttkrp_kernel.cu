@@ -72,21 +72,24 @@ __device__ __forceinline__ Vec<V> vzero() {
     return r;
 }
 
-// One lane's V columns of a factor row (read-only path; 256-bit or 128-bit load).
-// `lanep` = factor base + this lane's column offset; `word` = row index, bit 31 (run-end flag) ignored:
-// address = lanep + (word << 1) * (R * 2) bytes, one shift and one 32x32->64 multiply-add.
+// One lane's V columns of a factor row (read-only path; 128-bit or 256-bit load).
+// `base` = factor matrix (uniform), `word` = row index with bit 31 (run-end flag) ignored, `sub` = this
+// lane's slot inside the row.  The element offset (row * R/V + sub) is formed in 32 bits - the shift
+// drops the flag bit - and scaled by one 32x32->64 multiply-add on the uniform base, so a row address
+// costs two instructions and no per-lane pointer registers.  Needs dims[m] < 2^28 (api.cu check_shape).
 template <int V, int R>
-__device__ __forceinline__ Vec<V> ld_row(const float* __restrict__ lanep, uint32_t word) {
-    const float* p;
-    asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(p) : "r"(word << 1), "n"(R * 2), "l"(lanep));
+__device__ __forceinline__ Vec<V> ld_row(const float* __restrict__ base, uint32_t word, uint32_t sub) {
+    constexpr int SH = (R / V == 16) ? 4 : (R / V == 8) ? 3 : (R / V == 4) ? 2 : 1;      // log2(lanes per row)
+    const uint32_t off = (word << SH) + sub;
     Vec<V> r;
     if constexpr (V == 8) {
+        const float* p = base + (size_t)off * 8;
         asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                      : "=f"(r.p[0].x), "=f"(r.p[0].y), "=f"(r.p[1].x), "=f"(r.p[1].y), "=f"(r.p[2].x), "=f"(r.p[2].y),
                        "=f"(r.p[3].x), "=f"(r.p[3].y)
                      : "l"(p));
     } else {
-        const float4 v = __ldg(reinterpret_cast<const float4*>(p));
+        const float4 v = __ldg(reinterpret_cast<const float4*>(base) + off);
         r.p[0] = make_float2(v.x, v.y);
         r.p[1] = make_float2(v.z, v.w);
     }
@@ -250,11 +253,6 @@ __global__ void __launch_bounds__(kBlockThreads, Geo<N, R>::MINB) k_mttkrp(const
         }
     };
 
-    const float* facp[N];                                 // factor bases + this lane's column offset
-#pragma unroll
-    for (int l = 1; l < N; ++l) facp[l] = a.fac[l] + sub * V;
-    facp[0] = nullptr;
-
     Vec<V> t[NL];                                         // t[0] = output row accumulator
 #pragma unroll
     for (int l = 0; l < NL; ++l) t[l] = vzero<V>();
@@ -275,11 +273,11 @@ __global__ void __launch_bounds__(kBlockThreads, Geo<N, R>::MINB) k_mttkrp(const
             for (int l = 1; l < NL; ++l) w[l] |= kFlag;
             w[N - 1] &= kKeyMask;
         }
-        al[s] = ld_row<V, R>(facp[N - 1], w[N - 1]);
+        al[s] = ld_row<V, R>(a.fac[N - 1], w[N - 1], sub);
         uint32_t f = w[N - 1] >> 31;
 #pragma unroll
         for (int l = 1; l < NL; ++l) {
-            if (w[l] & kFlag) rb[l][s] = ld_row<V, R>(facp[l], w[l]);
+            if (w[l] & kFlag) rb[l][s] = ld_row<V, R>(a.fac[l], w[l], sub);
             f |= (w[l] >> 31) << l;
         }
         val[s] = __uint_as_float(w[N]);

@@ -21,39 +21,75 @@ struct FieldMap { int src[kMaxModes]; };   // out.field[l] = in.field[src[l]]
 // time the whole grid gathers from one source window that stays in L2, and every 64-byte DRAM
 // fetch is used completely; inside a group the destination positions ascend in long runs (the
 // layouts' key orders are chosen for that, build.cu choose_key_order), so the stores stay whole sectors.
+constexpr int kRemapPerThread = 4;      // independent gathers in flight per thread (the chain ord -> prev -> record is 3 loads deep)
+
 template <bool BLOCKED>
 __global__ void __launch_bounds__(256) k_remap3(const uint4* __restrict__ in, const uint32_t* __restrict__ prev,
                                                 const uint32_t* __restrict__ ord, const uint8_t* __restrict__ dflags,
                                                 uint4* __restrict__ out, int64_t nnz, int64_t nnz_pad, FieldMap fm) {
-    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= nnz_pad) return;
-    const int64_t j = (BLOCKED && t < nnz) ? (int64_t)__ldcs(ord + t) : t;   // padding positions are handled in place
-    const uint32_t src = BLOCKED ? __ldg(prev + (j < nnz ? j : nnz - 1)) : __ldcs(prev + (j < nnz ? j : nnz - 1));
-    const uint4 r = __ldg(in + src);
-    const uint32_t f[3] = {r.x & kKeyMask, r.y & kKeyMask, r.z & kKeyMask};
-    uint32_t k[3];
+    constexpr int U = kRemapPerThread;
+    const int64_t base = (int64_t)blockIdx.x * (256 * U) + threadIdx.x;
+    int64_t j[U];
+    uint32_t src[U], fl[U];
+    uint4 r[U];
 #pragma unroll
-    for (int l = 0; l < 3; ++l) k[l] = fm.src[l] == 0 ? f[0] : (fm.src[l] == 1 ? f[1] : f[2]);
-    apply_run_flags<3>(k, dflags[j]);
-    __stcs(out + j, make_uint4(k[0], k[1], k[2], j < nnz ? r.w : 0u));
+    for (int i = 0; i < U; ++i) {
+        const int64_t t = base + i * 256;
+        j[i] = (BLOCKED && t < nnz) ? (int64_t)__ldcs(ord + t) : t;          // padding positions are handled in place
+        if (t >= nnz_pad) j[i] = -1;
+    }
+#pragma unroll
+    for (int i = 0; i < U; ++i) {
+        const int64_t jj = j[i] < 0 ? 0 : (j[i] < nnz ? j[i] : nnz - 1);
+        src[i] = BLOCKED ? __ldg(prev + jj) : __ldcs(prev + jj);
+        fl[i] = j[i] < 0 ? 0u : dflags[j[i]];
+    }
+#pragma unroll
+    for (int i = 0; i < U; ++i) r[i] = __ldg(in + src[i]);
+#pragma unroll
+    for (int i = 0; i < U; ++i) {
+        if (j[i] < 0) continue;
+        const uint32_t f[3] = {r[i].x & kKeyMask, r[i].y & kKeyMask, r[i].z & kKeyMask};
+        uint32_t k[3];
+#pragma unroll
+        for (int l = 0; l < 3; ++l) k[l] = fm.src[l] == 0 ? f[0] : (fm.src[l] == 1 ? f[1] : f[2]);
+        apply_run_flags<3>(k, fl[i]);
+        __stcs(out + j[i], make_uint4(k[0], k[1], k[2], j[i] < nnz ? r[i].w : 0u));
+    }
 }
 
 template <int N, bool BLOCKED>
 __global__ void __launch_bounds__(256) k_remap(const uint32_t* __restrict__ in, const uint32_t* __restrict__ prev,
                                                const uint32_t* __restrict__ ord, const uint8_t* __restrict__ dflags,
                                                uint32_t* __restrict__ out, int64_t nnz, int64_t nnz_pad, FieldMap fm) {
-    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= nnz_pad) return;
-    const int64_t j = (BLOCKED && t < nnz) ? (int64_t)__ldcs(ord + t) : t;
-    const uint32_t* r = in + (size_t)__ldg(prev + (j < nnz ? j : nnz - 1)) * (N + 1);
-    uint32_t k[N];
+    constexpr int U = kRemapPerThread;
+    const int64_t base = (int64_t)blockIdx.x * (256 * U) + threadIdx.x;
+    int64_t j[U];
+    const uint32_t* r[U];
 #pragma unroll
-    for (int l = 0; l < N; ++l) k[l] = __ldg(r + fm.src[l]) & kKeyMask;
-    apply_run_flags<N>(k, dflags[j]);
-    uint32_t* o = out + (size_t)j * (N + 1);
+    for (int i = 0; i < U; ++i) {
+        const int64_t t = base + i * 256;
+        j[i] = (BLOCKED && t < nnz) ? (int64_t)__ldcs(ord + t) : t;
+        if (t >= nnz_pad) j[i] = -1;
+    }
 #pragma unroll
-    for (int l = 0; l < N; ++l) o[l] = k[l];
-    o[N] = j < nnz ? __ldg(r + N) : 0u;
+    for (int i = 0; i < U; ++i) {
+        const int64_t jj = j[i] < 0 ? 0 : (j[i] < nnz ? j[i] : nnz - 1);
+        r[i] = in + (size_t)__ldg(prev + jj) * (N + 1);
+    }
+#pragma unroll
+    for (int i = 0; i < U; ++i) {
+        if (j[i] < 0) continue;
+        uint32_t k[N];
+#pragma unroll
+        for (int l = 0; l < N; ++l) k[l] = __ldg(r[i] + fm.src[l]) & kKeyMask;
+        const uint32_t val = j[i] < nnz ? __ldg(r[i] + N) : 0u;
+        apply_run_flags<N>(k, dflags[j[i]]);
+        uint32_t* o = out + (size_t)j[i] * (N + 1);
+#pragma unroll
+        for (int l = 0; l < N; ++l) o[l] = k[l];
+        o[N] = val;
+    }
 }
 
 template <int N>
@@ -77,7 +113,7 @@ mttkrp_status_t launch_remap(mttkrp_handle_s* h, int from, cudaStream_t st) {
         for (int l = 0; l < kMaxModes; ++l) fm.src[l] = 0;
         for (int l = 0; l < N; ++l) fm.src[l] = h->mode[from].pos[h->mode[to].order[l]];
         const int64_t nnz_pad = h->num_shards * (int64_t)h->shard_nnz;
-        const unsigned grid = (unsigned)((nnz_pad + 255) / 256);
+        const unsigned grid = (unsigned)((nnz_pad + 256 * kRemapPerThread - 1) / (256 * kRemapPerThread));
         TimedLaunch tl(h->timing, kClsRemap, st);
         switch (N) {
             case 2: launch_remap_n<2>(h, from, to, grid, nnz_pad, fm, st); break;
