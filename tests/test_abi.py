@@ -54,6 +54,7 @@ def test_workspace_bytes_is_host_arithmetic(lib):
     ([10, 0, 3], 5, 0, 1),           # non-positive dim -> EINVAL
     ([10, 4, 3], -1, 0, 1),          # nnz < 0
     ([10, 4, 3], 2**31, 0, 3),       # nnz >= 2^31
+    ([10, 2**28, 3], 5, 0, 3),       # a dimension >= 2^28 (row offsets are formed in 32 bits)
     ([10, 4, 3], 5, 12, 3),          # bad max_rank
 ])
 def test_bad_shapes_are_rejected(lib, dims, nnz, rank, status):

@@ -190,6 +190,36 @@ def test_errors_are_reported(P):
     h.destroy()
 
 
+@pytest.mark.parametrize("order", ["revcyclic", "desc", "asc", "cyclic"])
+@pytest.mark.parametrize("blocked", ["0", "1"])
+def test_remap_walks_and_key_orders(P, monkeypatch, order, blocked):
+    # Every key-order policy and both remap walks (destination order / source-block order, with blocks
+    # small enough that the tensor spans many of them) obey the same contract: the permutation equals the
+    # oracle's stable sort by the reported key tuple, the remapped copy is that sorted COO, Y within tolerance.
+    monkeypatch.setenv("MTTKRP_KEY_ORDER", order)
+    monkeypatch.setenv("MTTKRP_REMAP_BLOCKED", blocked)
+    monkeypatch.setenv("MTTKRP_REMAP_BLOCK_LOG2", "12")
+    for cfg, nnz, R in [(1, 150_001, 32), (3, 90_007, 16), (4, 60_013, 8)]:
+        spec = W.CONFIGS[cfg].scaled(nnz)
+        t = W.generate_tensor(spec)
+        N = len(spec.dims)
+        worst, info = _run_case(P, spec.dims, t.idx, t.vals, R, seed=6, order_modes=list(range(N)) + [0, N - 1, 1])
+        assert info["remap_blocked"] == [int(blocked)] * N
+        if order == "revcyclic":
+            assert info["key_order"] == [[(d - j) % N for j in range(N)] for d in range(N)]
+
+
+def test_blocked_walk_is_chosen_from_measured_runs(P):
+    # Without overrides mttkrp_create measures the runs of both walks: small modes (long runs) -> blocked.
+    spec = W.CONFIGS[1].scaled(3_000_017)          # > 2 blocks of 2^20 records
+    t = W.generate_tensor(spec)
+    dev = torch.device("cuda:0")
+    h = P.Mttkrp(spec.dims, t.idx.to(dev), t.vals.to(dev))
+    info = h.info()
+    assert info["remap_blocked"] == [1, 1, 1] and min(info["remap_avg_run"]) >= 4
+    h.destroy()
+
+
 def _sample_rows(idx_d, dim, rng, k=48):
     """Heaviest rows, rows around shard boundaries' worth of mass, and random rows."""
     counts = torch.bincount(idx_d.long(), minlength=dim)
