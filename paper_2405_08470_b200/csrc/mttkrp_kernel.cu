@@ -30,6 +30,7 @@
 // nonzero are zeroed by k_zero_rows from the precomputed list, so `out` is fully overwritten
 // without a memset.
 #include <algorithm>
+#include <type_traits>
 #include "common.cuh"
 
 namespace mk {
@@ -140,7 +141,7 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 #ifndef MK_MINB          // resident blocks per SM the register allocation must allow; 0 = per-N default below.
 #define MK_MINB 0        // Measured on B200 (configs[1], configs[2]): occupancy beats deeper look-ahead.
 #endif
-template <int N, int R>
+template <int N, int R, bool DEEP>
 struct Geo {
     static constexpr int V = (MK_V8 && R >= 16) ? 8 : 4; // rank columns per lane
     static constexpr int LPN = R / V;                    // lanes per nonzero (group size)
@@ -151,12 +152,15 @@ struct Geo {
     static constexpr int SLOTW = (RECW + 3) / 4 * 4;     // ring slot words (16-byte multiple)
     static constexpr int K = (NPW * SLOTW <= 32) ? 8 : 4;  // records per group per ring stage
     static constexpr int STAGES = MK_STAGES;             // round r computing, r+1 landed, the rest in flight
-    static constexpr int D = (MK_D < K) ? MK_D : K / 2;  // gather look-ahead, in steps (K % D == 0)
+    // gather look-ahead, in steps (K % D == 0).  DEEP: twice the look-ahead at one block per SM less, for
+    // factor matrices that do not fit L2 (every gather that misses is a random HBM access).
+    static constexpr int D0 = (DEEP && N <= 3) ? 2 * MK_D : MK_D;
+    static constexpr int D = (D0 < K) ? D0 : K / 2;
     static constexpr int RING_WORDS = STAGES * K * NPW * SLOTW;        // per warp
     static constexpr int ENT_WORDS = 2 * NPW * R;                       // per warp: first/last partial rows
     static constexpr int WARP_WORDS = RING_WORDS > ENT_WORDS ? RING_WORDS : ENT_WORDS;
     static constexpr int NL = N - 1;                     // accumulator levels t[0..NL-1]
-    static constexpr int MINB = MK_MINB ? MK_MINB : (N <= 3 ? 5 : 3);
+    static constexpr int MINB = MK_MINB ? MK_MINB : (N <= 3 ? (DEEP ? 4 : 5) : 3);
     static constexpr int SMEM_BYTES = 4 * (WARPS * WARP_WORDS + WARPS * NPW * R + 2 * WARPS * R + WARPS * 2 * NPW + 2 * WARPS);
 };
 
@@ -187,9 +191,9 @@ __device__ __forceinline__ void merge_runs(const int* rows, const float* vecs, i
     if (cur_row >= 0) emit(cur_row, acc, run == 0, true);
 }
 
-template <int N, int R>
-__global__ void __launch_bounds__(kBlockThreads, Geo<N, R>::MINB) k_mttkrp(const KernelArgs<N> a) {
-    using Ge = Geo<N, R>;
+template <int N, int R, bool DEEP>
+__global__ void __launch_bounds__(kBlockThreads, Geo<N, R, DEEP>::MINB) k_mttkrp(const KernelArgs<N> a) {
+    using Ge = Geo<N, R, DEEP>;
     constexpr int V = Ge::V, LPN = Ge::LPN, NPW = Ge::NPW, WARPS = Ge::WARPS, G = Ge::G, K = Ge::K, D = Ge::D;
     constexpr int STAGES = Ge::STAGES, RECW = Ge::RECW, SLOTW = Ge::SLOTW, NL = Ge::NL;
     constexpr int ROWW = NPW * SLOTW;                     // ring words between consecutive records of a group
@@ -463,15 +467,28 @@ static mttkrp_status_t launch_nr(mttkrp_handle_s* h, int d, const float* const* 
         for (int l = 1; l < N; ++l) a.fac[l] = factors[mm.order[l]];
         a.out = out;
         a.carry = h->carry;
-        constexpr int smem = Geo<N, R>::SMEM_BYTES;
-        static bool attr_set = false;
-        if (!attr_set) {
-            MK_CUDA(cudaFuncSetAttribute(k_mttkrp<N, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-            attr_set = true;
-        }
-        {
+        // Factor matrices that overflow L2 (126 MB) turn gather misses into random HBM reads: use the
+        // variant with the deeper look-ahead (measured on configs[2]: 2.96 vs 3.19 ms per mode).
+        int64_t fac_bytes = 0;
+        for (int l = 1; l < N; ++l) fac_bytes += h->dims[mm.order[l]] * (int64_t)R * 4;
+        const bool deep = N <= 3 && fac_bytes > (96ll << 20);
+        auto launch = [&](auto deep_tag) -> mttkrp_status_t {
+            constexpr bool DEEP = decltype(deep_tag)::value;
+            constexpr int smem = Geo<N, R, DEEP>::SMEM_BYTES;
+            static bool attr_set = false;
+            if (!attr_set) {
+                MK_CUDA(cudaFuncSetAttribute(k_mttkrp<N, R, DEEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+                attr_set = true;
+            }
             TimedLaunch tl(h->timing, kClsMttkrp, st);
-            k_mttkrp<N, R><<<(unsigned)h->num_shards, kBlockThreads, smem, st>>>(a);
+            k_mttkrp<N, R, DEEP><<<(unsigned)h->num_shards, kBlockThreads, smem, st>>>(a);
+            return MTTKRP_OK;
+        };
+        if constexpr (N <= 3) {
+            if (deep) MK_TRY(launch(std::true_type{}));
+            else MK_TRY(launch(std::false_type{}));
+        } else {
+            MK_TRY(launch(std::false_type{}));
         }
         if (mm.n_chains > 0) {
             TimedLaunch tl(h->timing, kClsFixup, st);
