@@ -74,6 +74,21 @@ def test_tiny_tensors(P, dims, nnz, dup, R):
     _run_case(P, list(dims), t.idx, t.vals, R, seed=1)
 
 
+def test_hand_worked_golden(P):
+    # tests/golden/hand_worked_3mode.txt (PAPER.md:121 by hand); rank 2 is padded to the library's smallest
+    # rank with zero columns.  Small integers and halves: exact in fp32.
+    from conftest import load_golden
+    dims, idx, vals, factors, want = load_golden("hand_worked_3mode.txt")
+    dev = torch.device("cuda:0")
+    fac = [torch.from_numpy(np.pad(f, ((0, 0), (0, 6)))).to(dev) for f in factors]
+    h = P.Mttkrp(dims, torch.from_numpy(idx).to(dev), torch.from_numpy(vals).to(dev))
+    for d in [0, 1, 2, 1]:
+        Y = h.mttkrp_mode(d, fac).cpu().numpy()
+        np.testing.assert_array_equal(Y[:, :2].astype(np.float64), want[d])
+        assert np.all(Y[:, 2:] == 0)
+    h.destroy()
+
+
 @pytest.mark.parametrize("R", [8, 16, 32, 64])
 def test_config1_full(P, R):
     # BASELINE.json configs[0] at full size (R=16 is the config's rank; the others widen it).

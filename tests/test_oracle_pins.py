@@ -42,22 +42,15 @@ def brute_force(dims, idx, vals, factors, d):
 
 
 def test_hand_worked_example():
-    # C(i2,r) += val * A(i0,r) * B(i1,r), worked by hand for three nonzeros.
-    dims = (2, 3, 2)
-    idx = np.array([[0, 1, 0], [1, 2, 0], [0, 1, 1]], dtype=np.int32)   # (0,1,0)=2 (1,2,1)=3 (0,0,1)=-1
-    vals = np.array([2.0, 3.0, -1.0], dtype=np.float32)
-    A0 = np.array([[1, 2], [3, 4]], dtype=np.float32)
-    A1 = np.array([[1, 0], [0, 1], [2, 2]], dtype=np.float32)
-    A2 = np.array([[1, -1], [2, 0.5]], dtype=np.float32)
-    want = {
-        0: [[-2, -2], [12, 3]],             # 2*[0,1]*[1,-1] - [1,0]*[2,.5] ; 3*[2,2]*[2,.5]
-        1: [[-2, -1], [2, -4], [18, 6]],    # -[1,2]*[2,.5] ; 2*[1,2]*[1,-1] ; 3*[3,4]*[2,.5]
-        2: [[0, 4], [17, 24]],              # 2*[1,2]*[0,1] ; 3*[3,4]*[2,2] - [1,2]*[1,0]
-    }
+    # tests/golden/hand_worked_3mode.txt: PAPER.md:121 worked by hand for three nonzeros (exact in fp64).
+    from conftest import load_golden
+    dims, idx, vals, factors, want = load_golden("hand_worked_3mode.txt")
     for d in range(3):
-        Y, S = oracle.mttkrp_mode(dims, idx, vals, [A0, A1, A2], d)
-        np.testing.assert_array_equal(Y, np.array(want[d], dtype=np.float64))
+        Y, S = oracle.mttkrp_mode(dims, idx, vals, factors, d)
+        np.testing.assert_array_equal(Y, want[d])
         assert np.all(S >= np.abs(Y))
+        Yn, _ = oracle.mttkrp_numpy(dims, idx, vals, factors, d)
+        np.testing.assert_array_equal(Yn, want[d])
 
 
 @pytest.mark.parametrize("dims,nnz", TINY_SHAPES)
