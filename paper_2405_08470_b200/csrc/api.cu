@@ -19,7 +19,6 @@ void set_error(const char* fmt, ...) {
     va_end(ap);
 }
 
-void choose_key_order(int N, const int64_t* dims, int d, const char* env, int* order);   // build.cu
 
 static mttkrp_status_t check_shape(int nmodes, const int64_t* dims, int64_t nnz) {
     if (!dims) { set_error("dims is NULL"); return MTTKRP_EINVAL; }
@@ -67,8 +66,10 @@ mttkrp_status_t mttkrp_workspace_bytes(int nmodes, const int64_t* dims, int64_t 
     if (!bytes) { set_error("bytes is NULL"); return MTTKRP_EINVAL; }
     MK_TRY(check_shape(nmodes, dims, nnz));
     if (max_rank != 0 && !valid_rank(max_rank)) { set_error("max_rank %d not in {0,8,16,32,64}", max_rank); return MTTKRP_EUNSUPPORTED; }
+    LayoutPlan lp;
+    plan_layouts(nmodes, dims, nnz, &lp);
     WorkspacePlan p;
-    MK_TRY(plan_workspace(nmodes, dims, nnz, max_rank, &p));
+    MK_TRY(plan_workspace(nmodes, dims, nnz, max_rank, lp.rec_words, &p));
     *bytes = p.total;
     return MTTKRP_OK;
 }
@@ -84,8 +85,10 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
     if (!workspace) { set_error("workspace is NULL"); return MTTKRP_EWORKSPACE; }
     if (reinterpret_cast<uintptr_t>(workspace) & 255u) { set_error("workspace must be 256-byte aligned"); return MTTKRP_EWORKSPACE; }
     if (nnz > 0 && (!aligned16(idx) || !aligned16(vals))) { set_error("idx/vals must be 16-byte aligned"); return MTTKRP_EINVAL; }
+    LayoutPlan lp;
+    plan_layouts(nmodes, dims, nnz, &lp);
     WorkspacePlan p;
-    MK_TRY(plan_workspace(nmodes, dims, nnz, max_rank, &p));
+    MK_TRY(plan_workspace(nmodes, dims, nnz, max_rank, lp.rec_words, &p));
     if (workspace_bytes < p.total) {
         set_error("workspace %zu bytes < required %zu", workspace_bytes, p.total);
         return MTTKRP_EWORKSPACE;
@@ -100,7 +103,8 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
     h->N = nmodes;
     h->nnz = nnz;
     for (int m = 0; m < nmodes; ++m) h->dims[m] = dims[m];
-    h->rec_words = nmodes + 1;
+    h->rec_words = lp.rec_words;
+    h->packed = lp.packed;
     h->shard_nnz = p.shard_nnz;
     h->num_shards = p.num_shards;
     h->rec_cur = reinterpret_cast<uint32_t*>(ws + p.rec_a);
@@ -111,21 +115,10 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
     h->max_rank = max_rank;
     h->device = dev;
     h->timing = new (std::nothrow) Timing();
-    // Key order of the layouts (reading 4).  The default makes every remap a stable partition
-    // by one key, which the blocked remap turns into L2-resident gathers; that pays when the nonzeros a
-    // source block sends to one output row form runs of several records.  The expected run for mode d
-    // is nnz / (dims[d] * number of blocks); when most modes are too large for that, the size-ordered
-    // tuple (one remap of the cycle moves whole fibers) is the better choice.
-    const char* order_env = getenv("MTTKRP_KEY_ORDER");
-    if (!order_env) {
-        const double nblk = (double)((nnz >> 20) > 0 ? (nnz >> 20) : 1);
-        int good = 0;
-        for (int d = 0; d < nmodes; ++d) good += ((double)nnz / ((double)dims[d] * nblk) >= 1.0) ? 1 : 0;
-        order_env = (2 * good >= nmodes) ? "revcyclic" : "desc";
-    }
     for (int d = 0; d < nmodes; ++d) {
         ModeMeta& mm = h->mode[d];
-        choose_key_order(nmodes, dims, d, order_env, mm.order);
+        for (int l = 0; l < nmodes; ++l) mm.order[l] = lp.order[d][l];
+        mm.pk = lp.pk[d];
         for (int l = 0; l < nmodes; ++l) mm.pos[mm.order[l]] = l;
         mm.next = reinterpret_cast<uint32_t*>(ws + p.next[d]);
         mm.ord = reinterpret_cast<uint32_t*>(ws + p.ord[d]);
@@ -137,7 +130,7 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
             h->stage_out[d] = reinterpret_cast<float*>(ws + p.stage_out[d]);
         }
     }
-    h->bytes_held = (int64_t)(p.persistent_end + (size_t)(nmodes + 1) * 4 * (size_t)(p.num_shards * p.shard_nnz));
+    h->bytes_held = (int64_t)(p.persistent_end + (size_t)lp.rec_words * 4 * (size_t)(p.num_shards * p.shard_nnz));
     mttkrp_status_t s = build_format(h, p, ws, idx, vals, static_cast<cudaStream_t>(cuda_stream));
     if (s != MTTKRP_OK) { delete h->timing; delete h; return s; }
     *out = h;
@@ -258,7 +251,7 @@ mttkrp_status_t mttkrp_get_info(mttkrp_handle_t h, mttkrp_info_t* info) {
         bits += ceil_log2(h->dims[m]);
     }
     bits += (int64_t)h->N * ceil_log2(h->nnz > 1 ? h->nnz : 2);
-    info->record_bytes = 4 * (h->N + 1);
+    info->record_bytes = 4 * h->rec_words;
     info->shard_nnz = h->shard_nnz;
     info->num_shards = h->num_shards;
     info->bytes_held = h->bytes_held;

@@ -30,13 +30,13 @@ static int choose_shard_nnz(int64_t nnz) {
     return s;
 }
 
-mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_rank, WorkspacePlan* p) {
+mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_rank, int rec_words, WorkspacePlan* p) {
     memset(p, 0, sizeof(*p));
     const size_t n = (size_t)nnz;
     p->shard_nnz = choose_shard_nnz(nnz);
     p->num_shards = (nnz + p->shard_nnz - 1) / p->shard_nnz;
     // both tensor copies are padded to a whole number of shards (zero-valued copies of the last nonzero)
-    const size_t rec_bytes = (size_t)(N + 1) * 4 * (size_t)(p->num_shards * p->shard_nnz);
+    const size_t rec_bytes = (size_t)rec_words * 4 * (size_t)(p->num_shards * p->shard_nnz);
     size_t off = 0;
     p->rec_a = off; off = align_up(off + rec_bytes);
     for (int d = 0; d < N; ++d) { p->next[d] = off; off = align_up(off + 4 * n); }
@@ -310,6 +310,20 @@ __global__ void k_build_records(const int32_t* __restrict__ idx, const float* __
     r[N] = k < nnz ? __float_as_uint(vals[src]) : 0u;
 }
 
+// Packed variant (common.cuh PackDesc): one 16-byte record per nonzero.
+template <int N>
+__global__ void k_build_records_pk(const int32_t* __restrict__ idx, const float* __restrict__ vals,
+                                   const uint32_t* __restrict__ perm, const uint8_t* __restrict__ flags, int64_t nnz,
+                                   int64_t nnz_pad, OrderArg order, PackDesc pd, uint4* __restrict__ rec) {
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nnz_pad) return;
+    const uint32_t src = perm[k < nnz ? k : nnz - 1];
+    uint32_t key[N];
+#pragma unroll
+    for (int l = 0; l < N; ++l) key[l] = (uint32_t)idx[(size_t)order.v[l] * nnz + src];
+    rec[k] = pk_pack<N>(key, flags[k], k < nnz ? __float_as_uint(vals[src]) : 0u, pd);
+}
+
 // key[j] = map[j] >> shift (the source block of destination position j)
 __global__ void k_block_keys(const uint32_t* __restrict__ map, int shift, uint32_t* __restrict__ key, int64_t n) {
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -408,6 +422,38 @@ void choose_key_order(int N, const int64_t* dims, int d, const char* env, int* o
         });
     }
     for (int j = 0; j < n; ++j) order[j + 1] = rest[j];
+}
+
+void plan_layouts(int N, const int64_t* dims, int64_t nnz, LayoutPlan* lp) {
+    // Key order of the layouts (reading 4).  The default makes every remap a stable partition
+    // by one key, which the blocked remap turns into L2-resident gathers; that pays when the nonzeros a
+    // source block sends to one output row form runs of several records.  The expected run for mode d
+    // is nnz / (dims[d] * number of blocks); when most modes are too large for that, the size-ordered
+    // tuple (one remap of the cycle moves whole fibers) is the better choice.
+    const char* order_env = getenv("MTTKRP_KEY_ORDER");
+    if (!order_env) {
+        const double nblk = (double)((nnz >> 20) > 0 ? (nnz >> 20) : 1);
+        int good = 0;
+        for (int d = 0; d < N; ++d) good += ((double)nnz / ((double)dims[d] * nblk) >= 1.0) ? 1 : 0;
+        order_env = (2 * good >= N) ? "revcyclic" : "desc";
+    }
+    memset(lp, 0, sizeof(*lp));
+    for (int d = 0; d < N; ++d) choose_key_order(N, dims, d, order_env, lp->order[d]);
+    // Record format: packed 16-byte records for N >= 4 when every layout fits (common.cuh PackDesc).
+    const char* pack_env = getenv("MTTKRP_PACK");                 // 0 forces 4*(N+1)-byte records (tests)
+    bool packed = N >= 4 && !(pack_env && pack_env[0] == '0');
+    for (int d = 0; d < N && packed; ++d) {
+        int off = 0;
+        for (int l = 0; l < N; ++l) {
+            const int b = std::max(1, ceil_log2_i64(dims[lp->order[d][l]]));
+            lp->pk[d].bits[l] = b;
+            lp->pk[d].off[l] = (l < N - 1) ? off : 0;
+            if (l < N - 1) off += b;
+        }
+        if (off > 64 || lp->pk[d].bits[N - 1] + (N - 1) > 32) packed = false;
+    }
+    lp->packed = packed ? 1 : 0;
+    lp->rec_words = packed ? 4 : N + 1;
 }
 
 mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char* ws, const int32_t* idx,
@@ -512,7 +558,21 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
         OrderArg oa;
         for (int l = 0; l < kMaxModes; ++l) oa.v[l] = h->mode[0].order[l];
         const int64_t nnz_pad = nshards * (int64_t)S;
-        k_build_records<<<grid_for(nnz_pad, 256), 256, 0, st>>>(idx, vals, h->perm0, h->mode[0].lflags, nnz, nnz_pad, N, oa, h->rec_cur);
+        if (h->packed) {
+            uint4* rec = reinterpret_cast<uint4*>(h->rec_cur);
+            const unsigned g = grid_for(nnz_pad, 256);
+            const PackDesc pd = h->mode[0].pk;
+            switch (N) {
+                case 4: k_build_records_pk<4><<<g, 256, 0, st>>>(idx, vals, h->perm0, h->mode[0].lflags, nnz, nnz_pad, oa, pd, rec); break;
+                case 5: k_build_records_pk<5><<<g, 256, 0, st>>>(idx, vals, h->perm0, h->mode[0].lflags, nnz, nnz_pad, oa, pd, rec); break;
+                case 6: k_build_records_pk<6><<<g, 256, 0, st>>>(idx, vals, h->perm0, h->mode[0].lflags, nnz, nnz_pad, oa, pd, rec); break;
+                case 7: k_build_records_pk<7><<<g, 256, 0, st>>>(idx, vals, h->perm0, h->mode[0].lflags, nnz, nnz_pad, oa, pd, rec); break;
+                case 8: k_build_records_pk<8><<<g, 256, 0, st>>>(idx, vals, h->perm0, h->mode[0].lflags, nnz, nnz_pad, oa, pd, rec); break;
+                default: set_error("packed records need nmodes >= 4"); return MTTKRP_EINVAL;
+            }
+        } else {
+            k_build_records<<<grid_for(nnz_pad, 256), 256, 0, st>>>(idx, vals, h->perm0, h->mode[0].lflags, nnz, nnz_pad, N, oa, h->rec_cur);
+        }
         // Slot d still holds perm_d; go d = 0..N-1, the last one needs perm_0, which slot 0 no longer
         // holds -> use the perm0 copy.
         uint32_t* inv = keyA;
@@ -562,7 +622,7 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
         // fibers - the plain walk is already sequential on both sides).
         const int64_t runs = (int64_t)breaks[d] + 1;
         const int64_t src_runs = (int64_t)breaks[kMaxModes + d] + 1;
-        const bool fits = ((int64_t)(N + 1) * 4 << h->mode[d].block_log2) <= (48ll << 20);
+        const bool fits = ((int64_t)h->rec_words * 4 << h->mode[d].block_log2) <= (48ll << 20);
         bool blocked = nnz > 0 && fits && (nnz >> h->mode[d].block_log2) >= 2 && nnz / runs >= 4 &&
                        (double)nnz / (double)src_runs < 1.5;
         if (benv) blocked = nnz > 0 && benv[0] == '1';

@@ -49,10 +49,33 @@ __device__ __forceinline__ void apply_run_flags(uint32_t* k, uint32_t f) {
     k[N - 1] |= (f & 1u) << 31;
 }
 
+// Packed 16-byte records (N >= 4).  When the index widths allow, a record is {w0, w1, w2, val}: the keys of
+// levels 0..N-2 are a bit string in the 64 bits (w1:w0) (level l at bit off[l], bits[l] wide), the last
+// key sits in the low bits of w2 and the N-1 run-end flags in its top bits (e_l at bit 32-(N-1)+l).
+// This is the paper's bit-level size accounting applied to the hot-path record: the
+// remap then moves one 128-bit word per nonzero whatever N is.  Needs bits[N-1] + N-1 <= 32 and
+// sum_{l<N-1} bits[l] <= 64 in every layout; otherwise the handle keeps 4*(N+1)-byte records.
+struct PackDesc {
+    int32_t bits[kMaxModes];
+    int32_t off[kMaxModes];
+};
+__host__ __device__ __forceinline__ uint32_t pk_mask(int bits) { return bits >= 32 ? 0xffffffffu : ((1u << bits) - 1u); }
+__device__ __forceinline__ uint32_t pk_get(uint32_t w0, uint32_t w1, int off, uint32_t mask) {
+    return (uint32_t)(((((uint64_t)w1) << 32) | w0) >> off) & mask;
+}
+template <int N>
+__device__ __forceinline__ uint4 pk_pack(const uint32_t* k, uint32_t flags, uint32_t val, const PackDesc& d) {
+    uint64_t w01 = 0;
+#pragma unroll
+    for (int l = 0; l < N - 1; ++l) w01 |= (uint64_t)k[l] << d.off[l];
+    return make_uint4((uint32_t)w01, (uint32_t)(w01 >> 32), k[N - 1] | (flags << (32 - (N - 1))), val);
+}
+
 // Per-mode tables built by mttkrp_create.
 struct ModeMeta {
     int order[kMaxModes];     // sort-key order of this layout, order[0] == mode
     int pos[kMaxModes];       // pos[m] = level of mode m in `order`
+    PackDesc pk;              // bit layout of this layout's packed records (handle->packed)
     uint32_t* next;           // [nnz] gather map of the remap d -> (d+1)%N: position in THIS layout of the
                               // element at position j of the next layout (the paper's remap id, read backwards)
     uint32_t* ord;            // [nnz] positions of the NEXT layout ordered by the 2^block_log2-record block of this
@@ -99,7 +122,8 @@ struct mttkrp_handle_s {
     int N;
     int64_t dims[mk::kMaxModes];
     int64_t nnz;
-    int rec_words;            // N + 1 (N role-ordered int32 indices, then the fp32 value)
+    int rec_words;            // N + 1 (N role-ordered int32 indices, then the fp32 value), or 4 when packed
+    int packed;               // 1: 16-byte packed records (N >= 4 and the index widths fit, see PackDesc)
     int shard_nnz;
     int64_t num_shards;
     uint32_t* rec_cur;        // resident tensor copy T_in, layout `cur`
@@ -130,7 +154,15 @@ struct WorkspacePlan {
     int shard_nnz;
     int64_t num_shards;
 };
-mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_rank, WorkspacePlan* p);
+// Host-side choice of the layouts (key order per mode) and of the record format; pure arithmetic on the shape.
+struct LayoutPlan {
+    int order[kMaxModes][kMaxModes];
+    PackDesc pk[kMaxModes];
+    int packed;
+    int rec_words;
+};
+void plan_layouts(int N, const int64_t* dims, int64_t nnz, LayoutPlan* lp);
+mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_rank, int rec_words, WorkspacePlan* p);
 mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char* ws,
                              const int32_t* idx, const float* vals, cudaStream_t st);
 

@@ -43,6 +43,8 @@ struct KernelArgs {
     const float* fac[N];     // fac[l] = factor of the mode at key level l (fac[0] unused)
     float* out;
     float* carry;            // [2*num_shards][R]
+    uint32_t kmask[N];       // packed records (common.cuh PackDesc): mask and bit offset of the key of level l;
+    int32_t koff[N];         // kmask[0] also masks word 0 of unpacked records (all ones)
 };
 
 // ---- small PTX helpers ------------------------------------------------------------------------
@@ -141,14 +143,14 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 #ifndef MK_MINB          // resident blocks per SM the register allocation must allow; 0 = per-N default below.
 #define MK_MINB 0        // Measured on B200 (configs[1], configs[2]): occupancy beats deeper look-ahead.
 #endif
-template <int N, int R, bool DEEP>
+template <int N, int R, bool DEEP, bool PACKED>
 struct Geo {
     static constexpr int V = (MK_V8 && R >= 16) ? 8 : 4; // rank columns per lane
     static constexpr int LPN = R / V;                    // lanes per nonzero (group size)
     static constexpr int NPW = 32 / LPN;                 // groups per warp
     static constexpr int WARPS = kBlockThreads / 32;
     static constexpr int G = WARPS * NPW;                // groups per block
-    static constexpr int RECW = N + 1;                   // record words
+    static constexpr int RECW = PACKED ? 4 : N + 1;      // record words
     static constexpr int SLOTW = (RECW + 3) / 4 * 4;     // ring slot words (16-byte multiple)
     static constexpr int K = (NPW * SLOTW <= 32) ? 8 : 4;  // records per group per ring stage
     static constexpr int STAGES = MK_STAGES;             // round r computing, r+1 landed, the rest in flight
@@ -191,9 +193,9 @@ __device__ __forceinline__ void merge_runs(const int* rows, const float* vecs, i
     if (cur_row >= 0) emit(cur_row, acc, run == 0, true);
 }
 
-template <int N, int R, bool DEEP>
-__global__ void __launch_bounds__(kBlockThreads, Geo<N, R, DEEP>::MINB) k_mttkrp(const KernelArgs<N> a) {
-    using Ge = Geo<N, R, DEEP>;
+template <int N, int R, bool DEEP, bool PACKED>
+__global__ void __launch_bounds__(kBlockThreads, Geo<N, R, DEEP, PACKED>::MINB) k_mttkrp(const KernelArgs<N> a) {
+    using Ge = Geo<N, R, DEEP, PACKED>;
     constexpr int V = Ge::V, LPN = Ge::LPN, NPW = Ge::NPW, WARPS = Ge::WARPS, G = Ge::G, K = Ge::K, D = Ge::D;
     constexpr int STAGES = Ge::STAGES, RECW = Ge::RECW, SLOTW = Ge::SLOTW, NL = Ge::NL;
     constexpr int ROWW = NPW * SLOTW;                     // ring words between consecutive records of a group
@@ -272,20 +274,31 @@ __global__ void __launch_bounds__(kBlockThreads, Geo<N, R, DEEP>::MINB) k_mttkrp
     auto prefetch = [&](const uint32_t* slot, int s, bool chunk_last) {
         uint32_t w[SLOTW];
         read_slot(slot, w);
-        if (chunk_last) {
+        if constexpr (PACKED) {                           // {w0, w1, w2 = flags | last key, val}
+            uint32_t f = w[2] >> (32 - (N - 1));
+            if (chunk_last) f = (f | ((1u << NL) - 2u)) & ~1u;
+            al[s] = ld_row<V, R>(a.fac[N - 1], w[2] & a.kmask[N - 1], sub);
 #pragma unroll
-            for (int l = 1; l < NL; ++l) w[l] |= kFlag;
-            w[N - 1] &= kKeyMask;
-        }
-        al[s] = ld_row<V, R>(a.fac[N - 1], w[N - 1], sub);
-        uint32_t f = w[N - 1] >> 31;
+            for (int l = 1; l < NL; ++l)
+                if (f & (1u << l)) rb[l][s] = ld_row<V, R>(a.fac[l], pk_get(w[0], w[1], a.koff[l], a.kmask[l]), sub);
+            val[s] = __uint_as_float(w[3]);
+            fl[s] = f;
+        } else {
+            if (chunk_last) {
 #pragma unroll
-        for (int l = 1; l < NL; ++l) {
-            if (w[l] & kFlag) rb[l][s] = ld_row<V, R>(a.fac[l], w[l], sub);
-            f |= (w[l] >> 31) << l;
+                for (int l = 1; l < NL; ++l) w[l] |= kFlag;
+                w[N - 1] &= kKeyMask;
+            }
+            al[s] = ld_row<V, R>(a.fac[N - 1], w[N - 1], sub);
+            uint32_t f = w[N - 1] >> 31;
+#pragma unroll
+            for (int l = 1; l < NL; ++l) {
+                if (w[l] & kFlag) rb[l][s] = ld_row<V, R>(a.fac[l], w[l], sub);
+                f |= (w[l] >> 31) << l;
+            }
+            val[s] = __uint_as_float(w[N]);
+            fl[s] = f;
         }
-        val[s] = __uint_as_float(w[N]);
-        fl[s] = f;
     };
     // Arithmetic of one step (its record sits at `slot`).
     auto compute = [&](const uint32_t* slot, int s) {
@@ -299,7 +312,7 @@ __global__ void __launch_bounds__(kBlockThreads, Geo<N, R, DEEP>::MINB) k_mttkrp
             }
         }
         if (e & 1u) {                                     // an output row ends inside the chunk
-            const uint32_t row = slot[0];
+            const uint32_t row = slot[0] & a.kmask[0];
             if (seg == 0) {
                 vstore<V>(&s_first[warp][g][sub * V], t[0]);
                 if (sub == 0) s_erow[warp][2 * g] = (int)row;
@@ -334,7 +347,7 @@ __global__ void __launch_bounds__(kBlockThreads, Geo<N, R, DEEP>::MINB) k_mttkrp
         __syncwarp();                                     // everyone is done with round r's stage
     }
     cp_async_wait<0>();
-    const uint32_t last_row = ring_g[((nrounds - 1) % STAGES) * STAGEW + (K - 1) * ROWW];
+    const uint32_t last_row = ring_g[((nrounds - 1) % STAGES) * STAGEW + (K - 1) * ROWW] & a.kmask[0];
     __syncwarp();
     // chunk epilogue: the still-open row goes to the first (seg == 0) or last partial-row entry
     float* const s_last = reinterpret_cast<float*>(ring);               // [NPW][R], aliases the ring
@@ -391,7 +404,7 @@ __global__ void __launch_bounds__(kBlockThreads, Geo<N, R, DEEP>::MINB) k_mttkrp
 
     // level 2: merge the warps' partial rows; rows shared with a neighbouring shard go to the carry buffer
     if (warp == 0) {
-        auto key0_at = [&](int64_t pos) { return __ldg(a.rec + (size_t)pos * RECW); };   // word 0 carries no flag
+        auto key0_at = [&](int64_t pos) { return __ldg(a.rec + (size_t)pos * RECW) & a.kmask[0]; };   // k_0 sits in word 0
         const uint32_t first_row = key0_at(s_begin);
         const uint32_t end_row = key0_at(s_end - 1);
         const bool head_shared = s_begin > 0 && key0_at(s_begin - 1) == first_row;
@@ -472,23 +485,28 @@ static mttkrp_status_t launch_nr(mttkrp_handle_s* h, int d, const float* const* 
         int64_t fac_bytes = 0;
         for (int l = 1; l < N; ++l) fac_bytes += h->dims[mm.order[l]] * (int64_t)R * 4;
         const bool deep = N <= 3 && fac_bytes > (96ll << 20);
-        auto launch = [&](auto deep_tag) -> mttkrp_status_t {
+        for (int l = 0; l < N; ++l) { a.kmask[l] = 0xffffffffu; a.koff[l] = 0; }
+        if (h->packed)
+            for (int l = 0; l < N; ++l) { a.kmask[l] = pk_mask(mm.pk.bits[l]); a.koff[l] = mm.pk.off[l]; }
+        auto launch = [&](auto deep_tag, auto packed_tag) -> mttkrp_status_t {
             constexpr bool DEEP = decltype(deep_tag)::value;
-            constexpr int smem = Geo<N, R, DEEP>::SMEM_BYTES;
+            constexpr bool PACKED = decltype(packed_tag)::value;
+            constexpr int smem = Geo<N, R, DEEP, PACKED>::SMEM_BYTES;
             static bool attr_set = false;
             if (!attr_set) {
-                MK_CUDA(cudaFuncSetAttribute(k_mttkrp<N, R, DEEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+                MK_CUDA(cudaFuncSetAttribute(k_mttkrp<N, R, DEEP, PACKED>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
                 attr_set = true;
             }
             TimedLaunch tl(h->timing, kClsMttkrp, st);
-            k_mttkrp<N, R, DEEP><<<(unsigned)h->num_shards, kBlockThreads, smem, st>>>(a);
+            k_mttkrp<N, R, DEEP, PACKED><<<(unsigned)h->num_shards, kBlockThreads, smem, st>>>(a);
             return MTTKRP_OK;
         };
         if constexpr (N <= 3) {
-            if (deep) MK_TRY(launch(std::true_type{}));
-            else MK_TRY(launch(std::false_type{}));
+            if (deep) MK_TRY(launch(std::true_type{}, std::false_type{}));
+            else MK_TRY(launch(std::false_type{}, std::false_type{}));
         } else {
-            MK_TRY(launch(std::false_type{}));
+            if (h->packed) MK_TRY(launch(std::false_type{}, std::true_type{}));
+            else MK_TRY(launch(std::false_type{}, std::false_type{}));
         }
         if (mm.n_chains > 0) {
             TimedLaunch tl(h->timing, kClsFixup, st);

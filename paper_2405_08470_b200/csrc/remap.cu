@@ -92,6 +92,48 @@ __global__ void __launch_bounds__(256) k_remap(const uint32_t* __restrict__ in, 
     }
 }
 
+// Packed 16-byte records (common.cuh PackDesc), any N >= 4: one 128-bit load and store per nonzero.  The host
+// composes, per destination level, where its key sits in the SOURCE record (RemapPk), so the kernel unpacks
+// straight into destination order and repacks with the destination layout's offsets and flags.
+struct RemapPk {
+    int32_t soff[kMaxModes];      // bit offset of the source field in (w1:w0), or -1: it is the low field of w2
+    uint32_t smask[kMaxModes];
+};
+
+template <int N, bool BLOCKED>
+__global__ void __launch_bounds__(256) k_remap_pk(const uint4* __restrict__ in, const uint32_t* __restrict__ prev,
+                                                  const uint32_t* __restrict__ ord, const uint8_t* __restrict__ dflags,
+                                                  uint4* __restrict__ out, int64_t nnz, int64_t nnz_pad, RemapPk rp, PackDesc dd) {
+    constexpr int U = kRemapPerThread;
+    const int64_t base = (int64_t)blockIdx.x * (256 * U) + threadIdx.x;
+    int64_t j[U];
+    uint32_t src[U], fl[U];
+    uint4 r[U];
+#pragma unroll
+    for (int i = 0; i < U; ++i) {
+        const int64_t t = base + i * 256;
+        j[i] = (BLOCKED && t < nnz) ? (int64_t)__ldcs(ord + t) : t;
+        if (t >= nnz_pad) j[i] = -1;
+    }
+#pragma unroll
+    for (int i = 0; i < U; ++i) {
+        const int64_t jj = j[i] < 0 ? 0 : (j[i] < nnz ? j[i] : nnz - 1);
+        src[i] = BLOCKED ? __ldg(prev + jj) : __ldcs(prev + jj);
+        fl[i] = j[i] < 0 ? 0u : dflags[j[i]];
+    }
+#pragma unroll
+    for (int i = 0; i < U; ++i) r[i] = __ldg(in + src[i]);
+#pragma unroll
+    for (int i = 0; i < U; ++i) {
+        if (j[i] < 0) continue;
+        uint32_t k[N];
+#pragma unroll
+        for (int l = 0; l < N; ++l)
+            k[l] = rp.soff[l] < 0 ? (r[i].z & rp.smask[l]) : pk_get(r[i].x, r[i].y, rp.soff[l], rp.smask[l]);
+        __stcs(out + j[i], pk_pack<N>(k, fl[i], j[i] < nnz ? r[i].w : 0u, dd));
+    }
+}
+
 template <int N>
 static void launch_remap_n(mttkrp_handle_s* h, int from, int to, unsigned grid, int64_t nnz_pad, const FieldMap& fm, cudaStream_t st) {
     const ModeMeta& mf = h->mode[from];
@@ -100,6 +142,21 @@ static void launch_remap_n(mttkrp_handle_s* h, int from, int to, unsigned grid, 
         if (mf.blocked) k_remap3<true><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, mf.next, mf.ord, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, fm);
         else k_remap3<false><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, mf.next, mf.ord, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, fm);
     } else {
+        if constexpr (N >= 4) {
+            if (h->packed) {
+                RemapPk rp;
+                for (int l = 0; l < kMaxModes; ++l) { rp.soff[l] = 0; rp.smask[l] = 0; }
+                for (int l = 0; l < N; ++l) {
+                    const int sl = fm.src[l];
+                    rp.soff[l] = (sl == N - 1) ? -1 : mf.pk.off[sl];
+                    rp.smask[l] = pk_mask(mf.pk.bits[sl]);
+                }
+                const PackDesc dd = h->mode[to].pk;
+                if (mf.blocked) k_remap_pk<N, true><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, mf.next, mf.ord, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, rp, dd);
+                else k_remap_pk<N, false><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, mf.next, mf.ord, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, rp, dd);
+                return;
+            }
+        }
         if (mf.blocked) k_remap<N, true><<<grid, 256, 0, st>>>(h->rec_cur, mf.next, mf.ord, dflags, h->rec_alt, h->nnz, nnz_pad, fm);
         else k_remap<N, false><<<grid, 256, 0, st>>>(h->rec_cur, mf.next, mf.ord, dflags, h->rec_alt, h->nnz, nnz_pad, fm);
     }
@@ -161,11 +218,27 @@ __global__ void k_export(const uint32_t* __restrict__ rec, int64_t nnz, int N, P
     vals[k] = __uint_as_float(r[N]);
 }
 
+// packed records: pos.v[m] = level of mode m in the resident layout
+__global__ void k_export_pk(const uint4* __restrict__ rec, int64_t nnz, int N, PosArg pos, PackDesc pd,
+                            int32_t* __restrict__ idx, float* __restrict__ vals) {
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nnz) return;
+    const uint4 r = rec[k];
+    for (int m = 0; m < N; ++m) {
+        const int l = pos.v[m];
+        const uint32_t mask = pk_mask(pd.bits[l]);
+        idx[(size_t)m * nnz + k] = (int32_t)(l == N - 1 ? (r.z & mask) : pk_get(r.x, r.y, pd.off[l], mask));
+    }
+    vals[k] = __uint_as_float(r.w);
+}
+
 mttkrp_status_t launch_export(const mttkrp_handle_s* h, int32_t* idx, float* vals, cudaStream_t st) {
     if (h->nnz > 0) {
         PosArg pa;
         for (int m = 0; m < kMaxModes; ++m) pa.v[m] = h->mode[h->cur].pos[m];
-        k_export<<<(unsigned)((h->nnz + 255) / 256), 256, 0, st>>>(h->rec_cur, h->nnz, h->N, pa, idx, vals);
+        const unsigned grid = (unsigned)((h->nnz + 255) / 256);
+        if (h->packed) k_export_pk<<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, h->nnz, h->N, pa, h->mode[h->cur].pk, idx, vals);
+        else k_export<<<grid, 256, 0, st>>>(h->rec_cur, h->nnz, h->N, pa, idx, vals);
         MK_CUDA(cudaGetLastError());
     }
     return MTTKRP_OK;

@@ -224,6 +224,45 @@ def test_remap_walks_and_key_orders(P, monkeypatch, order, blocked):
             assert info["key_order"] == [[(d - j) % N for j in range(N)] for d in range(N)]
 
 
+@pytest.mark.parametrize("pack", ["0", "1"])
+def test_record_formats_for_four_and_more_modes(P, monkeypatch, pack):
+    # N >= 4: packed 16-byte records (bit-level layout) and the 4*(N+1)-byte fallback
+    # compute the same thing; both remap walks; record_bytes reports the format.
+    monkeypatch.setenv("MTTKRP_PACK", pack)
+    monkeypatch.setenv("MTTKRP_REMAP_BLOCK_LOG2", "12")
+    for dims, nnz, R in [((37, 50, 19, 64), 20_011, 32), ((9, 30, 1000, 7, 24), 30_013, 16),
+                         ((5, 4, 6, 3, 4, 5), 3_001, 8), ((3, 2, 4, 2, 3, 2, 5, 2), 2_003, 64)]:
+        spec = W.TensorSpec("fmt", list(dims), nnz, [1.1] + [0.0] * (len(dims) - 1), "uniform", (R,), 91)
+        t = W.generate_tensor(spec)
+        N = len(dims)
+        worst, info = _run_case(P, list(dims), t.idx, t.vals, R, seed=8, order_modes=list(range(N)) + [1, 0])
+        assert info["record_bytes"] == (16 if pack == "1" else 4 * (N + 1))
+
+
+def test_wide_index_tensor_falls_back_to_unpacked_records(P):
+    # 3 x 22 bits of leading keys do not fit the 64-bit key string: the handle keeps 20-byte records.
+    # (The cell count exceeds 64 bits, so the COO list is drawn directly; duplicates are legal and add.)
+    dims = [1 << 22, 1 << 22, 1 << 22, 1 << 10]
+    g = torch.Generator().manual_seed(92)
+    nnz = 50_021
+    idx = torch.stack([torch.randint(0, d, (nnz,), generator=g, dtype=torch.int64) for d in dims]).to(torch.int32)
+    vals = torch.rand(nnz, generator=g, dtype=torch.float32)
+    t = W.SparseTensor(W.TensorSpec("wide", dims, nnz, [0.0] * 4, "uniform", (8,), 92), idx, vals)
+    dev = torch.device("cuda:0")
+    h = P.Mttkrp(dims, t.idx.to(dev), t.vals.to(dev))
+    assert h.info()["record_bytes"] == 20
+    fac_np = [np.random.default_rng(m).uniform(-1, 1, size=(d, 8)).astype(np.float32) for m, d in enumerate(dims)]
+    fac = [torch.from_numpy(f).to(dev) for f in fac_np]
+    rng = np.random.default_rng(5)
+    for d in [0, 3]:
+        Y = h.mttkrp_mode(d, fac)
+        rows = np.unique(t.idx[d].numpy()[rng.choice(t.nnz, 64, replace=False)]).astype(np.int64)
+        Yo, So = oracle.mttkrp_rows(dims, t.idx.numpy(), t.vals.numpy(), fac_np, d, rows)
+        err, zeros_ok = oracle.normalised_error(Y[torch.from_numpy(rows).to(dev)].cpu().numpy(), Yo, So)
+        assert zeros_ok and err <= TOL
+    h.destroy()
+
+
 def test_blocked_walk_is_chosen_from_measured_runs(P):
     # Without overrides mttkrp_create measures the runs of both walks: small modes (long runs) -> blocked.
     spec = W.CONFIGS[1].scaled(3_000_017)          # > 2 blocks of 2^20 records
