@@ -162,7 +162,7 @@ struct Geo {
     static constexpr int ENT_WORDS = 2 * NPW * R;                       // per warp: first/last partial rows
     static constexpr int WARP_WORDS = RING_WORDS > ENT_WORDS ? RING_WORDS : ENT_WORDS;
     static constexpr int NL = N - 1;                     // accumulator levels t[0..NL-1]
-    static constexpr int MINB = MK_MINB ? MK_MINB : (N <= 3 ? (DEEP ? 4 : 5) : 3);
+    static constexpr int MINB = MK_MINB ? MK_MINB : (N <= 3 ? (DEEP ? 4 : 5) : (N == 4 ? 4 : 3));
     static constexpr int SMEM_BYTES = 4 * (WARPS * WARP_WORDS + WARPS * NPW * R + 2 * WARPS * R + WARPS * 2 * NPW + 2 * WARPS);
 };
 
