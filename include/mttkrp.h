@@ -123,8 +123,9 @@ mttkrp_status_t mttkrp_remap_to(mttkrp_handle_t h, int d, void* cuda_stream);
 /*
  * Same as mttkrp_sweep with HOST buffers: factors[m] host fp32 [dims[m]][R] (pinned memory makes
  * the copies asynchronous), outs[d] host fp32 [dims[d]][R].  Copies every factor to the
- * workspace staging area, runs all modes, copies every Y_d back, and synchronises the stream
- * before returning.  Needs max_rank >= R at create.
+ * workspace staging area, runs all modes, copies every Y_d back, and synchronises before
+ * returning.  The copies run on two internal streams so that they overlap the kernels (the
+ * kernels run on cuda_stream).  Needs max_rank >= R at create.
  */
 mttkrp_status_t mttkrp_sweep_host(mttkrp_handle_t h, const float* const* factors, int R,
                                   float* const* outs, void* cuda_stream);

@@ -181,16 +181,40 @@ mttkrp_status_t mttkrp_sweep_host(mttkrp_handle_t h, const float* const* factors
     for (int m = 0; m < h->N; ++m)
         if (!factors[m] || !outs[m]) { set_error("factors[%d]/outs[%d] is NULL", m, m); return MTTKRP_EINVAL; }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (!h->host_path_ready) {
+        MK_CUDA(cudaStreamCreateWithFlags(&h->s_in, cudaStreamNonBlocking));
+        MK_CUDA(cudaStreamCreateWithFlags(&h->s_out, cudaStreamNonBlocking));
+        for (int m = 0; m < h->N; ++m) {
+            MK_CUDA(cudaEventCreateWithFlags(&h->ev_in[m], cudaEventDisableTiming));
+            MK_CUDA(cudaEventCreateWithFlags(&h->ev_done[m], cudaEventDisableTiming));
+        }
+        MK_CUDA(cudaEventCreateWithFlags(&h->ev_sync, cudaEventDisableTiming));
+        h->host_path_ready = 1;
+    }
+    // Copies overlap the kernels: factors go in on one stream (A_0, which mode 0 does not read, last), every
+    // Y_d goes out on another while the next mode runs; the caller's stream carries the kernels.
     const float* dfac[kMaxModes];
-    for (int m = 0; m < h->N; ++m) {
-        MK_CUDA(cudaMemcpyAsync(h->stage_fac[m], factors[m], (size_t)h->dims[m] * R * 4, cudaMemcpyHostToDevice, st));
+    MK_CUDA(cudaEventRecord(h->ev_sync, st));
+    MK_CUDA(cudaStreamWaitEvent(h->s_in, h->ev_sync, 0));
+    for (int i = 0; i < h->N; ++i) {
+        const int m = (i + 1) % h->N;
+        MK_CUDA(cudaMemcpyAsync(h->stage_fac[m], factors[m], (size_t)h->dims[m] * R * 4, cudaMemcpyHostToDevice, h->s_in));
+        MK_CUDA(cudaEventRecord(h->ev_in[m], h->s_in));
         dfac[m] = h->stage_fac[m];
     }
     for (int d = 0; d < h->N; ++d) {
+        if (d == 0) {
+            for (int m = 1; m < h->N; ++m) MK_CUDA(cudaStreamWaitEvent(st, h->ev_in[m], 0));
+        } else if (d == 1) {
+            MK_CUDA(cudaStreamWaitEvent(st, h->ev_in[0], 0));
+        }
         MK_TRY(run_mode(h, d, dfac, R, h->stage_out[d], st));
-        MK_CUDA(cudaMemcpyAsync(outs[d], h->stage_out[d], (size_t)h->dims[d] * R * 4, cudaMemcpyDeviceToHost, st));
+        MK_CUDA(cudaEventRecord(h->ev_done[d], st));
+        MK_CUDA(cudaStreamWaitEvent(h->s_out, h->ev_done[d], 0));
+        MK_CUDA(cudaMemcpyAsync(outs[d], h->stage_out[d], (size_t)h->dims[d] * R * 4, cudaMemcpyDeviceToHost, h->s_out));
     }
     MK_CUDA(cudaStreamSynchronize(st));
+    MK_CUDA(cudaStreamSynchronize(h->s_out));
     return MTTKRP_OK;
 }
 
@@ -199,6 +223,12 @@ mttkrp_status_t mttkrp_destroy(mttkrp_handle_t h) {
     if (h->timing) {
         for (auto& e : h->timing->ev) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
         delete h->timing;
+    }
+    if (h->host_path_ready) {
+        for (int m = 0; m < h->N; ++m) { cudaEventDestroy(h->ev_in[m]); cudaEventDestroy(h->ev_done[m]); }
+        cudaEventDestroy(h->ev_sync);
+        cudaStreamDestroy(h->s_in);
+        cudaStreamDestroy(h->s_out);
     }
     delete h;
     return MTTKRP_OK;

@@ -139,6 +139,9 @@ struct mttkrp_handle_s {
     int64_t remaps_done;
     int device;
     mk::Timing* timing;       // owned; per-kernel event pairs while mttkrp_timing_begin is active
+    cudaStream_t s_in, s_out; // copy streams of mttkrp_sweep_host (created on first use)
+    cudaEvent_t ev_in[mk::kMaxModes], ev_done[mk::kMaxModes], ev_sync;
+    int host_path_ready;
 };
 
 namespace mk {

@@ -75,6 +75,15 @@ __device__ __forceinline__ Vec<V> vzero() {
     return r;
 }
 
+#ifndef MK_L2HINT        // 1: the record stream is read with an L2 evict-first policy, so that it does not push the
+#define MK_L2HINT 1      //    factor rows (the data that is re-used) out of L2 (measured: -2 % on configs[1], -1 % on
+                         //    configs[2]; an evict-last hint on the factor rows themselves was 10 % slower)
+#endif
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
 // One lane's V columns of a factor row (read-only path; 128-bit or 256-bit load).
 // `base` = factor matrix (uniform), `word` = row index with bit 31 (run-end flag) ignored, `sub` = this
 // lane's slot inside the row.  The element offset (row * R/V + sub) is formed in 32 bits - the shift
@@ -117,8 +126,13 @@ __device__ __forceinline__ void vstore(float* dst, const Vec<V>& v) {
         *reinterpret_cast<float4*>(dst + 4 * i) = make_float4(v.p[2 * i].x, v.p[2 * i].y, v.p[2 * i + 1].x, v.p[2 * i + 1].y);
 }
 
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, uint64_t policy) {
+#if MK_L2HINT
+    asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "l"(policy) : "memory");
+#else
+    (void)policy;
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+#endif
 }
 __device__ __forceinline__ void cp_async8(uint32_t dst, const void* src) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
@@ -232,6 +246,7 @@ __global__ void __launch_bounds__(kBlockThreads, Geo<N, R, DEEP, PACKED>::MINB) 
     const uint32_t* const ring_g = ring + g * SLOTW;      // this group's column of the ring
     const uint32_t ring_gs = (uint32_t)__cvta_generic_to_shared(ring_g);
 
+    const uint64_t rec_policy = l2_policy_evict_first();
     auto issue_round = [&](int r) {
         if (r < nrounds) {
             const uint32_t* src = grec + (size_t)r * (K * RECW);
@@ -242,7 +257,7 @@ __global__ void __launch_bounds__(kBlockThreads, Geo<N, R, DEEP, PACKED>::MINB) 
                 if (p < K * PPR) {
                     const int jj = p / PPR, q = p % PPR;
                     const uint32_t d2 = dst + 4u * (uint32_t)(jj * ROWW + q * PW);
-                    if constexpr (PW == 4) cp_async16(d2, src + jj * RECW + q * PW);
+                    if constexpr (PW == 4) cp_async16(d2, src + jj * RECW + q * PW, rec_policy);
                     else if constexpr (PW == 2) cp_async8(d2, src + jj * RECW + q * PW);
                     else cp_async4(d2, src + jj * RECW + q * PW);
                 }
