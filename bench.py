@@ -42,6 +42,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-sample-nnz", type=int, default=32_000_000)
+    ap.add_argument("--partition-report", action="store_true",
+                    help="also run the paper's Alg. 1 partitioner (kappa = 148) and report its load balance")
     return ap.parse_args()
 
 
@@ -300,6 +302,16 @@ def run_ours(args):
                "h2d_bytes_per_step": io, "d2h_bytes_per_step": io, "ms_per_step": ms_e2e / args.steps,
                "api": "mttkrp_sweep_host (pinned host factors in, pinned host Y_d out)"}
 
+    partition = None
+    if args.partition_report:
+        # Alg. 1 with one partition per SM: whole rows, longest first.  Equal-nnz shards are
+        # balanced by construction (max/mean = 1); this shows what indivisible rows cost on the same tensor.
+        partition = {"kappa": 148, "max_over_mean": []}
+        for d in range(N):
+            _, loads = h.partition_rows(d, 148)
+            partition["max_over_mean"].append(round(float(loads.max()) / (float(loads.sum()) / 148), 3))
+        partition["note"] = "paper's Alg. 1 (whole rows, longest-first) on the same tensor; this library's equal-nnz shards: 1.0"
+
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu_baseline, _, _ = time_oracle_sample(spec, R, sample_n, tensor_cpu)
@@ -319,7 +331,7 @@ def run_ours(args):
                            "bytes_held": info["bytes_held"], "bytes_paper_format": info["bytes_paper_format"],
                            "create_s": t_create, "generate_s": t_gen},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_sweep * args.steps,
-                "roofline": roofline, "breakdown": breakdown, "cpu_baseline": cpu_baseline,
+                "roofline": roofline, "breakdown": breakdown, "cpu_baseline": cpu_baseline, "partition": partition,
                 "paper_context": "geomean speedups 1.5x / 2.0x / 21.7x over BLCO / MM-CSF / ParTI-GPU on RTX 3090 "
                                  "(PAPER.md:414); no absolute numbers published"}
         print(json.dumps(line), flush=True)

@@ -162,6 +162,24 @@ typedef struct {
 mttkrp_status_t mttkrp_timing_begin(mttkrp_handle_t h);
 mttkrp_status_t mttkrp_timing_end(mttkrp_handle_t h, mttkrp_timing_t* out /*host*/, void* cuda_stream);
 
+/*
+ * The paper's tensor partitioning scheme for one mode (Alg. 1), as an analysis tool: the
+ * output rows of mode d ("vertices", with degree = number of nonzeros in the row) are ordered by descending
+ * degree (ties: lower index first) and dealt one by one to the currently least-loaded of kappa partitions
+ * (ties: lowest partition id) - the longest-first rule behind the 4/3 bound the paper cites (
+ * DESIGN.md reading 3: the algorithm's body is missing from the paper's text).  Whole rows only (Observation 2,
+ * PAPER.md:301-303).  This library does NOT shard this way (it splits heavy rows, reading 13); the
+ * call exists to compare the two policies.
+ *   deg_dev:  device int32 [dims[d]], scratch, receives the row degrees (computed on the device from the
+ *             resident tensor copy; asynchronous work is synchronised before the host part runs).
+ *   part_of_row: host int32 [dims[d]] or NULL, receives the partition of every row.
+ *   loads:    host int64 [kappa], receives the nonzeros per partition.
+ * Errors: EINVAL (null pointers, kappa < 1, d out of range), ECUDA.
+ */
+mttkrp_status_t mttkrp_partition_rows(mttkrp_handle_t h, int d, int kappa, int32_t* deg_dev /*device*/,
+                                      int32_t* part_of_row /*host, may be NULL*/, int64_t* loads /*host*/,
+                                      void* cuda_stream);
+
 /* Library / build identification, e.g. "mttkrp_b200 0.1 sm_100a". */
 const char* mttkrp_version(void);
 

@@ -22,7 +22,7 @@ _STATUS_NAMES = {0: "MTTKRP_OK", 1: "MTTKRP_EINVAL", 2: "MTTKRP_EINDEX", 3: "MTT
 
 EXPORTS = ["mttkrp_workspace_bytes", "mttkrp_create", "mttkrp_mode", "mttkrp_sweep", "mttkrp_remap_to",
            "mttkrp_sweep_host", "mttkrp_destroy", "mttkrp_last_error", "mttkrp_get_info", "mttkrp_get_perm",
-           "mttkrp_export_coo", "mttkrp_timing_begin", "mttkrp_timing_end", "mttkrp_version"]
+           "mttkrp_export_coo", "mttkrp_timing_begin", "mttkrp_timing_end", "mttkrp_partition_rows", "mttkrp_version"]
 
 
 class MttkrpError(RuntimeError):
@@ -72,6 +72,7 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.mttkrp_get_info.argtypes = [vp, ctypes.POINTER(Info)]
     lib.mttkrp_get_perm.argtypes = [vp, ctypes.c_int, vp, vp, vp]
     lib.mttkrp_export_coo.argtypes = [vp, vp, vp, vp]
+    lib.mttkrp_partition_rows.argtypes = [vp, ctypes.c_int, ctypes.c_int, vp, vp, vp, vp]
     lib.mttkrp_timing_begin.argtypes = [vp]
     lib.mttkrp_timing_end.argtypes = [vp, ctypes.POINTER(Timing), vp]
     for name in EXPORTS:
@@ -216,6 +217,17 @@ class Mttkrp:
             "key_order": [list(raw.key_order[d])[:n] for d in range(n)],
             "remap_blocked": list(raw.remap_blocked)[:n], "remap_avg_run": list(raw.remap_avg_run)[:n],
         }
+
+    def partition_rows(self, d: int, kappa: int):
+        """Alg. 1 of the paper for mode d: (partition of every row [int32, host], nonzeros per partition [int64])."""
+        import numpy as np
+        deg = torch.empty(int(self.dims[d]), dtype=torch.int32, device=self.device)
+        part = np.empty(int(self.dims[d]), dtype=np.int32)
+        loads = np.empty(int(kappa), dtype=np.int64)
+        with torch.cuda.device(self.device):
+            _check(load_library().mttkrp_partition_rows(self._h, int(d), int(kappa), deg.data_ptr(),
+                                                        part.ctypes.data, loads.ctypes.data, _stream()))
+        return part, loads
 
     def get_perm(self, d: int) -> torch.Tensor:
         perm = torch.empty(max(self.nnz, 1), dtype=torch.int32, device=self.device)

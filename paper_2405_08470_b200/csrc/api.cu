@@ -5,7 +5,11 @@
 #include <cstdlib>
 #include <cstdlib>
 #include <cstring>
+#include <algorithm>
 #include <new>
+#include <queue>
+#include <utility>
+#include <vector>
 #include "common.cuh"
 
 namespace mk {
@@ -312,6 +316,37 @@ mttkrp_status_t mttkrp_export_coo(mttkrp_handle_t h, int32_t* idx_dev, float* va
     if (h->nnz == 0) return MTTKRP_OK;
     if (!idx_dev || !vals_dev) { set_error("idx/vals is NULL"); return MTTKRP_EINVAL; }
     return launch_export(h, idx_dev, vals_dev, static_cast<cudaStream_t>(cuda_stream));
+}
+
+mttkrp_status_t mttkrp_partition_rows(mttkrp_handle_t h, int d, int kappa, int32_t* deg_dev, int32_t* part_of_row,
+                                      int64_t* loads, void* cuda_stream) {
+    if (!h) { set_error("handle is NULL"); return MTTKRP_EINVAL; }
+    if (d < 0 || d >= h->N) { set_error("mode %d outside [0,%d)", d, h->N); return MTTKRP_EINVAL; }
+    if (kappa < 1) { set_error("kappa %d < 1", kappa); return MTTKRP_EINVAL; }
+    if (!deg_dev || !loads) { set_error("deg_dev/loads is NULL"); return MTTKRP_EINVAL; }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    MK_TRY(launch_row_degrees(h, d, deg_dev, st));
+    const int64_t rows = h->dims[d];
+    std::vector<int32_t> deg((size_t)rows);
+    MK_CUDA(cudaMemcpyAsync(deg.data(), deg_dev, sizeof(int32_t) * (size_t)rows, cudaMemcpyDeviceToHost, st));
+    MK_CUDA(cudaStreamSynchronize(st));
+    // Alg. 1: vertices by descending degree, each to the least-loaded partition.
+    std::vector<int32_t> order((size_t)rows);
+    for (int64_t i = 0; i < rows; ++i) order[(size_t)i] = (int32_t)i;
+    std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) { return deg[(size_t)a] > deg[(size_t)b]; });
+    typedef std::pair<int64_t, int> Bin;                       // (load, partition id): min-heap, ties to the lowest id
+    std::priority_queue<Bin, std::vector<Bin>, std::greater<Bin>> heap;
+    for (int z = 0; z < kappa; ++z) { loads[z] = 0; heap.push(Bin(0, z)); }
+    for (int64_t q = 0; q < rows; ++q) {
+        const int32_t v = order[(size_t)q];
+        Bin b = heap.top();
+        heap.pop();
+        b.first += deg[(size_t)v];
+        loads[b.second] = b.first;
+        if (part_of_row) part_of_row[v] = b.second;
+        heap.push(b);
+    }
+    return MTTKRP_OK;
 }
 
 }  // extern "C"

@@ -172,6 +172,7 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
 // ---- remap.cu -------------------------------------------------------------------------------
 mttkrp_status_t launch_remap(mttkrp_handle_s* h, int from, cudaStream_t st);   // from -> (from+1)%N, swaps copies
 mttkrp_status_t launch_export(const mttkrp_handle_s* h, int32_t* idx, float* vals, cudaStream_t st);
+mttkrp_status_t launch_row_degrees(const mttkrp_handle_s* h, int d, int32_t* deg_dev, cudaStream_t st);
 mttkrp_status_t launch_perm_step(const uint32_t* map, const uint32_t* in, uint32_t* out, int64_t nnz, cudaStream_t st);
 
 // ---- mttkrp_kernel.cu -----------------------------------------------------------------------

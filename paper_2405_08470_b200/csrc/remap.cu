@@ -244,4 +244,28 @@ mttkrp_status_t launch_export(const mttkrp_handle_s* h, int32_t* idx, float* val
     return MTTKRP_OK;
 }
 
+// Row degrees of one mode from the resident copy (Alg. 1's vertex degrees): level = position of
+// that mode in the resident layout's key order.  Off the hot path; global atomics are fine here.
+__global__ void k_row_degrees(const uint32_t* __restrict__ rec, int64_t nnz, int rec_words, int packed, int N, int level,
+                              PackDesc pd, int32_t* __restrict__ deg) {
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nnz) return;
+    const uint32_t* r = rec + (size_t)k * rec_words;
+    uint32_t key;
+    if (packed) key = level == N - 1 ? (r[2] & pk_mask(pd.bits[level])) : pk_get(r[0], r[1], pd.off[level], pk_mask(pd.bits[level]));
+    else key = r[level] & kKeyMask;
+    atomicAdd(deg + key, 1);
+}
+
+mttkrp_status_t launch_row_degrees(const mttkrp_handle_s* h, int d, int32_t* deg_dev, cudaStream_t st) {
+    MK_CUDA(cudaMemsetAsync(deg_dev, 0, sizeof(int32_t) * (size_t)h->dims[d], st));
+    if (h->nnz > 0) {
+        const ModeMeta& mm = h->mode[h->cur];
+        k_row_degrees<<<(unsigned)((h->nnz + 255) / 256), 256, 0, st>>>(h->rec_cur, h->nnz, h->rec_words, h->packed, h->N,
+                                                                         mm.pos[d], mm.pk, deg_dev);
+        MK_CUDA(cudaGetLastError());
+    }
+    return MTTKRP_OK;
+}
+
 }  // namespace mk

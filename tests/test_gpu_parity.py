@@ -50,7 +50,8 @@ def _run_case(P, dims, idx_cpu, vals_cpu, R, seed, order_modes=None, check_perm=
     modes = list(order_modes) if order_modes is not None else list(range(N))
     worst = 0.0
     for d in modes:
-        Y = h.mttkrp_mode(d, fac).cpu().numpy()
+        out = torch.full((dims[d], R), float("nan"), dtype=torch.float32, device=dev)   # every entry must be overwritten
+        Y = h.mttkrp_mode(d, fac, out=out).cpu().numpy()
         assert h.info()["cur_layout"] == d
         if d in perms:                                                # remapped copy is the sorted COO
             gi, gv = h.export_coo()
