@@ -507,11 +507,8 @@ static mttkrp_status_t launch_nr(mttkrp_handle_s* h, int d, const float* const* 
             constexpr bool DEEP = decltype(deep_tag)::value;
             constexpr bool PACKED = decltype(packed_tag)::value;
             constexpr int smem = Geo<N, R, DEEP, PACKED>::SMEM_BYTES;
-            static bool attr_set = false;
-            if (!attr_set) {
+            if constexpr (smem > 48 * 1024)               // per device, so not cached in a static
                 MK_CUDA(cudaFuncSetAttribute(k_mttkrp<N, R, DEEP, PACKED>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-                attr_set = true;
-            }
             TimedLaunch tl(h->timing, kClsMttkrp, st);
             k_mttkrp<N, R, DEEP, PACKED><<<(unsigned)h->num_shards, kBlockThreads, smem, st>>>(a);
             return MTTKRP_OK;

@@ -232,7 +232,8 @@ def test_record_formats_for_four_and_more_modes(P, monkeypatch, pack):
     monkeypatch.setenv("MTTKRP_PACK", pack)
     monkeypatch.setenv("MTTKRP_REMAP_BLOCK_LOG2", "12")
     for dims, nnz, R in [((37, 50, 19, 64), 20_011, 32), ((9, 30, 1000, 7, 24), 30_013, 16),
-                         ((5, 4, 6, 3, 4, 5), 3_001, 8), ((3, 2, 4, 2, 3, 2, 5, 2), 2_003, 64)]:
+                         ((5, 4, 6, 3, 4, 5), 3_001, 8), ((3, 2, 4, 2, 3, 2, 5, 2), 2_003, 64),
+                         ((3, 2, 4, 2, 3, 2, 5, 2), 2_003, 8)]:     # unpacked: > 48 KB of shared memory per block
         spec = W.TensorSpec("fmt", list(dims), nnz, [1.1] + [0.0] * (len(dims) - 1), "uniform", (R,), 91)
         t = W.generate_tensor(spec)
         N = len(dims)
