@@ -126,6 +126,7 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
         for (int l = 0; l < nmodes; ++l) mm.pos[mm.order[l]] = l;
         mm.next = reinterpret_cast<uint32_t*>(ws + p.next[d]);
         mm.ord = reinterpret_cast<uint32_t*>(ws + p.ord[d]);
+        mm.osrc = reinterpret_cast<uint32_t*>(ws + p.osrc[d]);
         mm.lflags = reinterpret_cast<uint8_t*>(ws + p.lflags[d]);
         mm.empty_rows = reinterpret_cast<uint32_t*>(ws + p.empty[d]);
         mm.chains = reinterpret_cast<uint32_t*>(ws + p.chains[d]);

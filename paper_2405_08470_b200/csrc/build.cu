@@ -41,6 +41,7 @@ mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_
     p->rec_a = off; off = align_up(off + rec_bytes);
     for (int d = 0; d < N; ++d) { p->next[d] = off; off = align_up(off + 4 * n); }
     for (int d = 0; d < N; ++d) { p->ord[d] = off; off = align_up(off + 4 * n); }
+    for (int d = 0; d < N; ++d) { p->osrc[d] = off; off = align_up(off + 4 * n); }
     for (int d = 0; d < N; ++d) { p->lflags[d] = off; off = align_up(off + (size_t)(p->num_shards * p->shard_nnz)); }
     p->perm0 = off; off = align_up(off + 4 * n);
     for (int d = 0; d < N; ++d) { p->empty[d] = off; off = align_up(off + 4 * (size_t)dims[d]); }
@@ -602,6 +603,7 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
             k_radix_hist<<<(unsigned)nblocks, kSortThreads, 0, st>>>(keyA, nnz, 0, hist, nblocks);
             MK_TRY(exclusive_scan(hist, 256 * nblocks, sums, st));
             k_radix_scatter<<<(unsigned)nblocks, kSortThreads, 0, st>>>(keyA, permA, keyB, mm.ord, nnz, 0, hist, nblocks);
+            k_gather_u32<<<grid_for(nnz, 256), 256, 0, st>>>(mm.next, mm.ord, mm.osrc, nnz);
             k_count_breaks<<<grid_for(nnz, 256), 256, 0, st>>>(mm.ord, nnz, small + 32 + d);
             k_count_breaks<<<grid_for(nnz, 256), 256, 0, st>>>(mm.next, nnz, small + 40 + d);
         }

@@ -81,6 +81,8 @@ struct ModeMeta {
     uint32_t* ord;            // [nnz] positions of the NEXT layout ordered by the 2^block_log2-record block of this
                               // layout they come from (stable), or unused: the blocked remap walks the destination
                               // in this order so that its random reads stay inside one L2-resident window at a time
+    uint32_t* osrc;           // [nnz] osrc[t] = next[ord[t]]: the source position of walk step t (saves the walk one
+                              // dependent gather)
     int blocked;              // 1: the remap d -> (d+1)%N uses `ord`
     int block_log2;
     double avg_run;           // average length of the ascending destination runs in `ord`
@@ -149,7 +151,7 @@ namespace mk {
 // ---- build.cu -------------------------------------------------------------------------------
 struct WorkspacePlan {
     size_t rec_a, rec_b, perm0, carry;
-    size_t next[kMaxModes], empty[kMaxModes], chains[kMaxModes], ord[kMaxModes], lflags[kMaxModes];
+    size_t next[kMaxModes], empty[kMaxModes], chains[kMaxModes], ord[kMaxModes], osrc[kMaxModes], lflags[kMaxModes];
     size_t stage_fac[kMaxModes], stage_out[kMaxModes];
     size_t persistent_end;
     size_t scratch;          // start of the create-time scratch (may overlap rec_b)

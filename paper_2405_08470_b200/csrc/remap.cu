@@ -25,8 +25,9 @@ constexpr int kRemapPerThread = 4;      // independent gathers in flight per thr
 
 template <bool BLOCKED>
 __global__ void __launch_bounds__(256) k_remap3(const uint4* __restrict__ in, const uint32_t* __restrict__ prev,
-                                                const uint32_t* __restrict__ ord, const uint8_t* __restrict__ dflags,
-                                                uint4* __restrict__ out, int64_t nnz, int64_t nnz_pad, FieldMap fm) {
+                                                const uint32_t* __restrict__ ord, const uint32_t* __restrict__ osrc,
+                                                const uint8_t* __restrict__ dflags, uint4* __restrict__ out, int64_t nnz,
+                                                int64_t nnz_pad, FieldMap fm) {
     constexpr int U = kRemapPerThread;
     const int64_t base = (int64_t)blockIdx.x * (256 * U) + threadIdx.x;
     int64_t j[U];
@@ -37,13 +38,11 @@ __global__ void __launch_bounds__(256) k_remap3(const uint4* __restrict__ in, co
         const int64_t t = base + i * 256;
         j[i] = (BLOCKED && t < nnz) ? (int64_t)__ldcs(ord + t) : t;          // padding positions are handled in place
         if (t >= nnz_pad) j[i] = -1;
+        if (BLOCKED && t < nnz) src[i] = __ldcs(osrc + t);
+        else src[i] = __ldcs(prev + (t < nnz ? t : nnz - 1));
     }
 #pragma unroll
-    for (int i = 0; i < U; ++i) {
-        const int64_t jj = j[i] < 0 ? 0 : (j[i] < nnz ? j[i] : nnz - 1);
-        src[i] = BLOCKED ? __ldg(prev + jj) : __ldcs(prev + jj);
-        fl[i] = j[i] < 0 ? 0u : dflags[j[i]];
-    }
+    for (int i = 0; i < U; ++i) fl[i] = j[i] < 0 ? 0u : dflags[j[i]];
 #pragma unroll
     for (int i = 0; i < U; ++i) r[i] = __ldg(in + src[i]);
 #pragma unroll
@@ -102,8 +101,9 @@ struct RemapPk {
 
 template <int N, bool BLOCKED>
 __global__ void __launch_bounds__(256) k_remap_pk(const uint4* __restrict__ in, const uint32_t* __restrict__ prev,
-                                                  const uint32_t* __restrict__ ord, const uint8_t* __restrict__ dflags,
-                                                  uint4* __restrict__ out, int64_t nnz, int64_t nnz_pad, RemapPk rp, PackDesc dd) {
+                                                  const uint32_t* __restrict__ ord, const uint32_t* __restrict__ osrc,
+                                                  const uint8_t* __restrict__ dflags, uint4* __restrict__ out, int64_t nnz,
+                                                  int64_t nnz_pad, RemapPk rp, PackDesc dd) {
     constexpr int U = kRemapPerThread;
     const int64_t base = (int64_t)blockIdx.x * (256 * U) + threadIdx.x;
     int64_t j[U];
@@ -114,13 +114,11 @@ __global__ void __launch_bounds__(256) k_remap_pk(const uint4* __restrict__ in, 
         const int64_t t = base + i * 256;
         j[i] = (BLOCKED && t < nnz) ? (int64_t)__ldcs(ord + t) : t;
         if (t >= nnz_pad) j[i] = -1;
+        if (BLOCKED && t < nnz) src[i] = __ldcs(osrc + t);
+        else src[i] = __ldcs(prev + (t < nnz ? t : nnz - 1));
     }
 #pragma unroll
-    for (int i = 0; i < U; ++i) {
-        const int64_t jj = j[i] < 0 ? 0 : (j[i] < nnz ? j[i] : nnz - 1);
-        src[i] = BLOCKED ? __ldg(prev + jj) : __ldcs(prev + jj);
-        fl[i] = j[i] < 0 ? 0u : dflags[j[i]];
-    }
+    for (int i = 0; i < U; ++i) fl[i] = j[i] < 0 ? 0u : dflags[j[i]];
 #pragma unroll
     for (int i = 0; i < U; ++i) r[i] = __ldg(in + src[i]);
 #pragma unroll
@@ -139,8 +137,8 @@ static void launch_remap_n(mttkrp_handle_s* h, int from, int to, unsigned grid, 
     const ModeMeta& mf = h->mode[from];
     const uint8_t* dflags = h->mode[to].lflags;
     if constexpr (N == 3) {
-        if (mf.blocked) k_remap3<true><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, mf.next, mf.ord, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, fm);
-        else k_remap3<false><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, mf.next, mf.ord, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, fm);
+        if (mf.blocked) k_remap3<true><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, mf.next, mf.ord, mf.osrc, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, fm);
+        else k_remap3<false><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, mf.next, mf.ord, mf.osrc, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, fm);
     } else {
         if constexpr (N >= 4) {
             if (h->packed) {
@@ -152,8 +150,8 @@ static void launch_remap_n(mttkrp_handle_s* h, int from, int to, unsigned grid, 
                     rp.smask[l] = pk_mask(mf.pk.bits[sl]);
                 }
                 const PackDesc dd = h->mode[to].pk;
-                if (mf.blocked) k_remap_pk<N, true><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, mf.next, mf.ord, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, rp, dd);
-                else k_remap_pk<N, false><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, mf.next, mf.ord, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, rp, dd);
+                if (mf.blocked) k_remap_pk<N, true><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, mf.next, mf.ord, mf.osrc, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, rp, dd);
+                else k_remap_pk<N, false><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, mf.next, mf.ord, mf.osrc, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, rp, dd);
                 return;
             }
         }
