@@ -21,14 +21,17 @@ struct FieldMap { int src[kMaxModes]; };   // out.field[l] = in.field[src[l]]
 // time the whole grid gathers from one source window that stays in L2, and every 64-byte DRAM
 // fetch is used completely; inside a group the destination positions ascend in long runs (the
 // layouts' key orders are chosen for that, build.cu choose_key_order), so the stores stay whole sectors.
-constexpr int kRemapPerThread = 4;      // independent gathers in flight per thread (the chain ord -> prev -> record is 3 loads deep)
+// Independent gather chains in flight per thread: 4 for the blocked walk (L2 hits), 8 for the plain walk (random
+// HBM reads need more parallelism); measured on configs[1] / configs[2].
+template <bool BLOCKED>
+__host__ __device__ constexpr int remap_per_thread() { return BLOCKED ? 4 : 8; }
 
 template <bool BLOCKED>
 __global__ void __launch_bounds__(256) k_remap3(const uint4* __restrict__ in, const uint32_t* __restrict__ prev,
                                                 const uint32_t* __restrict__ ord, const uint32_t* __restrict__ osrc,
                                                 const uint8_t* __restrict__ dflags, uint4* __restrict__ out, int64_t nnz,
                                                 int64_t nnz_pad, FieldMap fm) {
-    constexpr int U = kRemapPerThread;
+    constexpr int U = remap_per_thread<BLOCKED>();
     const int64_t base = (int64_t)blockIdx.x * (256 * U) + threadIdx.x;
     int64_t j[U];
     uint32_t src[U], fl[U];
@@ -61,7 +64,7 @@ template <int N, bool BLOCKED>
 __global__ void __launch_bounds__(256) k_remap(const uint32_t* __restrict__ in, const uint32_t* __restrict__ prev,
                                                const uint32_t* __restrict__ ord, const uint8_t* __restrict__ dflags,
                                                uint32_t* __restrict__ out, int64_t nnz, int64_t nnz_pad, FieldMap fm) {
-    constexpr int U = kRemapPerThread;
+    constexpr int U = remap_per_thread<BLOCKED>();
     const int64_t base = (int64_t)blockIdx.x * (256 * U) + threadIdx.x;
     int64_t j[U];
     const uint32_t* r[U];
@@ -104,7 +107,7 @@ __global__ void __launch_bounds__(256) k_remap_pk(const uint4* __restrict__ in, 
                                                   const uint32_t* __restrict__ ord, const uint32_t* __restrict__ osrc,
                                                   const uint8_t* __restrict__ dflags, uint4* __restrict__ out, int64_t nnz,
                                                   int64_t nnz_pad, RemapPk rp, PackDesc dd) {
-    constexpr int U = kRemapPerThread;
+    constexpr int U = remap_per_thread<BLOCKED>();
     const int64_t base = (int64_t)blockIdx.x * (256 * U) + threadIdx.x;
     int64_t j[U];
     uint32_t src[U], fl[U];
@@ -168,7 +171,8 @@ mttkrp_status_t launch_remap(mttkrp_handle_s* h, int from, cudaStream_t st) {
         for (int l = 0; l < kMaxModes; ++l) fm.src[l] = 0;
         for (int l = 0; l < N; ++l) fm.src[l] = h->mode[from].pos[h->mode[to].order[l]];
         const int64_t nnz_pad = h->num_shards * (int64_t)h->shard_nnz;
-        const unsigned grid = (unsigned)((nnz_pad + 256 * kRemapPerThread - 1) / (256 * kRemapPerThread));
+        const int per_block = 256 * (h->mode[from].blocked ? remap_per_thread<true>() : remap_per_thread<false>());
+        const unsigned grid = (unsigned)((nnz_pad + per_block - 1) / per_block);
         TimedLaunch tl(h->timing, kClsRemap, st);
         switch (N) {
             case 2: launch_remap_n<2>(h, from, to, grid, nnz_pad, fm, st); break;
