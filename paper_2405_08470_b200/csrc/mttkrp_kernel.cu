@@ -3,9 +3,10 @@
 // library's own, made for sm_100a).
 //
 // Layout: records sorted by the key tuple (k_0 = i_d, k_1, ..., k_{N-1}); record = N uint32 keys in
-// that order + fp32 value.  Bit 31 of the key words carries the run-end flags that the format builder
-// and the remap pass derived from the sorted order (common.cuh), so a record is self-contained: the
-// hot loop has no look-ahead compare.
+// that order + fp32 value, or (N >= 4, PACKED) 16 bytes with the keys bit-packed (common.cuh PackDesc).
+// The record carries the run-end flags that the format builder and the remap pass derived from the
+// sorted order (bit 31 of the key words / top bits of w2, common.cuh), so it is self-contained: the hot
+// loop has no look-ahead compare.
 // A thread block owns one shard = shard_nnz consecutive records (equal-nnz shards).  Inside the
 // block a GROUP of R/V lanes (V = 4 rank columns per lane, one 128-bit LDG per factor row per lane:
 // a warp instruction then covers whole 128-byte lines, one L1 wavefront each) walks a contiguous

@@ -3,7 +3,7 @@
 // destination (Observation 1).  Here the same permutation is applied in gather
 // form, T_out[j] = T_in[prev[j]]: stores are coalesced and whole 32-byte sectors, the random side is
 // the 16-byte loads.  On B200 the scatter form measured 2.3x slower (partial-sector writes turn
-// into read-modify-write in DRAM; profiles/r1_v1_ncu_summary.md).
+// into read-modify-write in DRAM; kernel v1 of round 1).
 // Records are role-ordered (sort keys major to minor, then the value), so the pass also permutes
 // the index fields from the source layout's key order to the destination's, refreshes the
 // zero-valued padding records that fill the last shard, and merges the destination layout's
