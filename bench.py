@@ -262,16 +262,19 @@ def run_ours(args):
         peak, peak_src = FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
     alg_bytes_launch = sum(bytes_mode) / N
     achieved = alg_bytes_launch / (k_ms * 1e-3) / 1e9 if k_ms > 0 else 0.0
-    traffic = None                                     # ncu dram bytes per launch of that kernel (profiles/r1_traffic.csv)
+    traffic = l2_hit = l1_hit = None                   # ncu figures of that kernel, per launch (profiles/r1_traffic.csv)
     tpath = os.path.join(ROOT, "profiles", "r1_traffic.csv")
     if os.path.exists(tpath):
         import csv
         for row in csv.DictReader(open(tpath)):
             if row["config"] == str(args.config) and row["kernel"] == "k_mttkrp" and not args.nnz and not args.rank:
                 traffic = float(row["dram_bytes_per_launch"])
+                l2_hit, l1_hit = float(row["l2_hit_pct"]), float(row["l1_hit_pct"])
     total_k = tm["remap_ms"] + tm["zero_ms"] + tm["mttkrp_ms"] + tm["fixup_ms"]
     roofline = {"bound": "hbm", "kernel": "k_mttkrp", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                "l2_hit_pct_ncu": l2_hit, "l1_hit_pct_ncu": l1_hit,
+                "dram_GBs_ncu": (traffic / (k_ms * 1e-3) / 1e9) if (traffic and k_ms > 0) else None,
                 "frac_of_nominal_8TBs": achieved / 8000.0,
                 "algorithmic_bytes_per_launch": alg_bytes_launch, "avg_launch_ms": k_ms,
                 "per_mode_algorithmic_bytes": bytes_mode}
