@@ -5,10 +5,12 @@
 
 A "step" is one steady-state sweep of the whole hot path over the resident tensor: for every mode
 d = 0..N-1 the remap into the mode-d layout (Alg. 3), the MTTKRP kernels (Alg. 2/4) and the split-row
-fix-up, i.e. N remaps + N MTTKRPs (Alg. 5).  Workload: BASELINE.json configs[C]
-(default C=1: 3-mode, 12,000 x 9,000 x 29,000, 77M nonzeros, Zipf 1.1, R=32), synthetic, seeded
-(`workloads/`).  `--gpus N` runs N independent replicas (replicas only, no
-collective on the data path).  One JSON line on stdout (rank 0).
+fix-up, i.e. N remaps + N MTTKRPs (Alg. 5).  Workload: BASELINE.json configs[C],
+default C=2 (the config BASELINE.md Sec. 2 quotes the target on: 3-mode, 4.8M x 1.8M x 1.8M, 200M
+nonzeros, Zipf 1.3/1.05/1.05, R=32), synthetic, seeded (`workloads/`).  The other configs and the rank
+sweep of configs[4] are measured in the same run and reported under `extra`.  `--gpus N` runs N
+independent replicas (replicas only, no collective on the data path).
+One JSON line on stdout (rank 0).
 """
 from __future__ import annotations
 
@@ -28,27 +30,45 @@ if ROOT not in sys.path:
 METRIC = "all-mode spMTTKRP GFLOP/s (nnz*N*R flops per mode, remap included)"
 UNIT = "GFLOP/s"
 FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback
+TRAFFIC_CSV = os.path.join("profiles", "r2_traffic.csv")   # ncu dram bytes per launch of the committed build
 
 
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (0-based)")
+    ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (0-based)")
     ap.add_argument("--rank", type=int, default=0, help="R (0 = the config's)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--nnz", type=int, default=0, help="override nnz (debug / scaled runs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--cpu-sample-nnz", type=int, default=32_000_000)
+    ap.add_argument("--no-extra", action="store_true", help="skip the other configs / rank sweep")
+    ap.add_argument("--cpu-sample-nnz", type=int, default=0,
+                    help="nonzeros the oracle legs process (prefix of the workload's shuffled COO list); "
+                         "0 = the whole workload for cpu_baseline, 8M per step for --impl reference")
     ap.add_argument("--partition-report", action="store_true",
-                    help="also run the paper's Alg. 1 partitioner (kappa = 148) and report its load balance")
+                    help="also run the paper's Alg. 1 partitioner (kappa = SM count) and report its load balance")
     return ap.parse_args()
+
+
+def default_rank(spec):
+    return spec.ranks[-1 if len(spec.ranks) == 1 else 2]
 
 
 def workload_name(spec, R):
     return f"configs[{spec.config_id - 1}] {spec.name} dims={'x'.join(str(d) for d in spec.dims)} nnz={spec.nnz} R={R}"
+
+
+def config_block(spec, R):
+    """Identical in both arms (`--impl ours` / `--impl reference`): names the workload, nothing else."""
+    N = len(spec.dims)
+    copy_mb = spec.nnz * 16 / 1e6
+    l2 = (f"inputs larger than L2: two tensor copies of {copy_mb:.0f} MB alternate (L2 is 126 MB)" if 2 * copy_mb > 126 else
+          f"inputs smaller than L2 ({copy_mb:.1f} MB per tensor copy): a launch-bound parity case, not a bench workload")
+    return {"workload": workload_name(spec, R), "nmodes": N, "nnz": spec.nnz, "R": R,
+            "step": f"one sweep = {N} remaps + {N} MTTKRPs over the resident tensor", "l2": l2}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -111,39 +131,60 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------
 # the oracle legs (the only places bench.py may execute oracle/)
 # ------------------------------------------------------------------------------------------------
-def time_oracle_sample(spec, R, sample_nnz, tensor_cpu=None):
-    """Times the fp64 oracle, as it stands, on the first `sample_nnz` nonzeros of the workload
-    (all modes: stable sort by the output index + accumulation), all host cores.  GFLOP/s with the
-    same flop convention."""
+def oracle_pass(dims, idx, vals, fac, R, perms=None):
+    """One pass of the fp64 oracle, as it stands, over the given nonzeros: for every mode the stable sort by
+    the output index (oracle.sort_perm, one thread) and the accumulation in sorted order with the rows split
+    across all host cores (oracle.mttkrp_mode).  Returns (accumulation seconds, sort seconds, perms).  The
+    sort is the oracle's format build; like mttkrp_create on the GPU side it is timed separately."""
+    import oracle
+    N = len(dims)
+    threads = max(oracle.max_threads(), 2)
+    t_sort = t_acc = 0.0
+    out_perms = []
+    for d in range(N):
+        if perms is None:
+            t0 = time.perf_counter()
+            perm = oracle.sort_perm(dims, idx, [d])
+            t_sort += time.perf_counter() - t0
+        else:
+            perm = perms[d]
+        out_perms.append(perm if perms is not None else None)
+        t0 = time.perf_counter()
+        oracle.mttkrp_mode(dims, idx, vals, fac, d, perm=perm, threads=threads)
+        t_acc += time.perf_counter() - t0
+        if perms is None:
+            del perm
+    return t_acc, t_sort, out_perms
+
+
+def cpu_baseline_leg(spec, R, idx, vals, fac_np, sample_nnz):
     import numpy as np
     import oracle
-    import workloads as W
-    if tensor_cpu is None:
-        sub = spec.scaled(min(sample_nnz, spec.nnz))
-        t = W.generate_tensor(sub)
-        idx, vals = t.idx.numpy(), t.vals.numpy()
-        what = f"{sub.nnz} nonzeros drawn from the workload's distribution (same dims and skew)"
-    else:
-        idx, vals = tensor_cpu
-        idx = np.ascontiguousarray(idx[:, :sample_nnz])
-        vals = np.ascontiguousarray(vals[:sample_nnz])
-        what = f"first {vals.shape[0]} nonzeros of the workload's (shuffled) COO list"
-    nnz = int(vals.shape[0])
-    N = len(spec.dims)
-    fac = [f.numpy() for f in W.generate_factors(spec, R)]
-    threads = oracle.max_threads()
     oracle.build()
-    t0 = time.perf_counter()
-    for d in range(N):
-        perm = oracle.sort_perm(spec.dims, idx, [d])
-        oracle.mttkrp_mode(spec.dims, idx, vals, fac, d, perm=perm, threads=max(threads, 2))
-    dt = time.perf_counter() - t0
-    flops = float(nnz) * N * R * N
-    return {"value": flops / dt / 1e9, "unit": UNIT, "cores": threads, "kind": "oracle",
-            "sample": f"{what}, all {N} modes, stable sort + fp64 accumulation, {dt:.2f} s"}, dt, nnz
+    nnz_all = int(vals.shape[0])
+    n = nnz_all if sample_nnz <= 0 else min(sample_nnz, nnz_all)
+    if n < nnz_all:
+        idx = np.ascontiguousarray(idx[:, :n])
+        vals = np.ascontiguousarray(vals[:n])
+        what = f"first {n} of the workload's {nnz_all} nonzeros (the COO list is in seeded random order)"
+    else:
+        what = f"the whole workload ({n} nonzeros)"
+    N = len(spec.dims)
+    t_acc, t_sort, _ = oracle_pass(spec.dims, idx, vals, fac_np, R)
+    flops = float(n) * N * R * N
+    return {"value": flops / t_acc / 1e9, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
+            "sample": f"{what}, all {N} modes, fp64 oracle as it stands (not a tuned CPU implementation): accumulation "
+                      f"{t_acc:.2f} s on all cores; its one-thread stable sort ({t_sort:.2f} s) is its format build and, "
+                      f"like mttkrp_create on the GPU side, is not in the figure",
+            "accumulate_s": t_acc, "sort_s": t_sort, "sample_nnz": n}
 
 
 def run_reference(args):
+    """--impl reference: the oracle on the host cores, on the SAME seeded tensor as the CUDA arm; every step is one
+    oracle pass over a bounded sample (a prefix of the shuffled COO list) so that K+W steps end within minutes."""
+    import numpy as np
+    import torch
+    import oracle
     import workloads as W
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -151,24 +192,30 @@ def run_reference(args):
     spec = W.CONFIGS[args.config]
     if args.nnz:
         spec = spec.scaled(args.nnz)
-    R = args.rank or spec.ranks[-1 if len(spec.ranks) == 1 else 2]
+    R = args.rank or default_rank(spec)
     N = len(spec.dims)
-    sample = min(args.cpu_sample_nnz // 4, spec.nnz)
+    gen_dev = "cuda" if torch.cuda.is_available() else "cpu"      # input generation only (workloads/ is shared)
+    t = W.generate_tensor(spec, gen_dev)
+    n = min(args.cpu_sample_nnz or 8_000_000, spec.nnz)
+    idx = np.ascontiguousarray(t.idx[:, :n].cpu().numpy())
+    vals = np.ascontiguousarray(t.vals[:n].cpu().numpy())
+    del t
+    fac = [f.numpy() for f in W.generate_factors(spec, R)]
+    oracle.build()
+    perms = [oracle.sort_perm(spec.dims, idx, [d]) for d in range(N)]       # the oracle's format build, once
     times = []
-    base = None
-    tcpu = W.generate_tensor(spec.scaled(sample))
-    tensor_cpu = (tcpu.idx.numpy(), tcpu.vals.numpy())
     for i in range(args.warmup + args.steps):
-        base, dt, nnz = time_oracle_sample(spec, R, sample, tensor_cpu)
+        t_acc, _, _ = oracle_pass(spec.dims, idx, vals, fac, R, perms)
         if i >= args.warmup:
-            times.append(dt)
+            times.append(t_acc)
     ms = 1e3 * sum(times) / len(times)
-    value = float(nnz) * N * R * N / (ms / 1e3) / 1e9
-    base["value"] = value
+    value = float(n) * N * R * N / (ms / 1e3) / 1e9
+    base = {"value": value, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
+            "sample": f"every step = the fp64 oracle over the first {n} of the workload's {spec.nnz} nonzeros (seeded random "
+                      f"order), all {N} modes, pre-sorted once (as the CUDA arm excludes mttkrp_create)", "sample_nnz": n}
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic", "config": {"workload": workload_name(spec, R), "sample_nnz": nnz},
-            "cpu_baseline": base,
+            "dtype": "f64", "data": "synthetic", "config": config_block(spec, R), "cpu_baseline": base,
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -177,6 +224,136 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 # the CUDA arm
 # ------------------------------------------------------------------------------------------------
+def hbm_peak():
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(peaks_path):
+        return float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(config_id, R):
+    """dram bytes per k_mttkrp launch from the committed ncu capture of this build (profiles/r2_traffic.csv);
+    a constant of the committed profile, not measured by this run - None when no capture matches."""
+    path = os.path.join(ROOT, TRAFFIC_CSV)
+    if not os.path.exists(path):
+        return None
+    import csv
+    for row in csv.DictReader(open(path)):
+        if row["config"] == str(config_id) and row["kernel"] == "k_mttkrp" and int(row.get("R", 32)) == R:
+            return {"traffic": float(row["dram_bytes_per_launch"]), "l2_hit_pct": float(row["l2_hit_pct"]),
+                    "l1_hit_pct": float(row["l1_hit_pct"]), "source": TRAFFIC_CSV}
+    return None
+
+
+class Case:
+    """One workload resident on the device: tensor handle, factors, outputs, byte model."""
+
+    def __init__(self, P, W, spec, R, dev, max_rank, keep_coo=False):
+        import torch
+        self.spec, self.R, self.dev = spec, R, dev
+        self.N = len(spec.dims)
+        t0 = time.perf_counter()
+        t = W.generate_tensor(spec, dev)
+        self.U = W.distinct_per_mode(t)
+        torch.cuda.synchronize()
+        self.generate_s = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        self.h = P.Mttkrp(spec.dims, t.idx, t.vals, max_rank=max_rank)
+        torch.cuda.synchronize()
+        self.create_s = time.perf_counter() - t0
+        self.checksums = t.checksums
+        self.nnz = t.nnz
+        self.coo = (t.idx.cpu().numpy(), t.vals.cpu().numpy()) if keep_coo else None
+        del t
+        torch.cuda.empty_cache()
+        self.info = self.h.info()
+        self.set_rank(W, R)
+
+    def set_rank(self, W, R):
+        import torch
+        self.R = R
+        self.fac = W.generate_factors(self.spec, R, self.dev)
+        self.outs = [torch.empty((d, R), dtype=torch.float32, device=self.dev) for d in self.spec.dims]
+        nnz, N, rec = self.nnz, self.N, self.info["record_bytes"]
+        self.flops_per_sweep = float(nnz) * N * R * N
+        self.bytes_mode = [nnz * rec + sum(self.U[m] for m in range(N) if m != d) * R * 4 + self.spec.dims[d] * R * 4
+                           for d in range(N)]
+        self.remap_bytes_mode = nnz * (2 * rec + 4 + 1)
+        info = self.info
+        # launches of OUR kernels per sweep: remap + zero-fill (if any empty row) + mttkrp + fix-up (if any split row)
+        self.launches_per_sweep = sum(2 + (1 if info["num_empty_rows"][d] else 0) + (1 if info["num_split_rows"][d] else 0)
+                                      for d in range(N)) if nnz else N
+
+    def sweep(self):
+        self.h.mttkrp_sweep(self.fac, self.outs)
+
+    def timed_sweeps(self, steps, barrier=None):
+        import torch
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        if barrier:
+            barrier()
+        w0 = time.time()
+        e0.record()
+        for _ in range(steps):
+            self.sweep()
+        e1.record()
+        if barrier:
+            barrier()
+        else:
+            torch.cuda.synchronize()
+        return e0.elapsed_time(e1), w0, time.time()
+
+    def kernel_classes(self, steps):
+        """Per-kernel-class device time: CUDA event pairs recorded inside the library on the launching stream."""
+        self.h.timing_begin()
+        for _ in range(steps):
+            self.sweep()
+        tm = self.h.timing_end()
+        k_ms = tm["mttkrp_ms"] / max(1, tm["mttkrp_launches"])
+        total_k = tm["remap_ms"] + tm["zero_ms"] + tm["mttkrp_ms"] + tm["fixup_ms"]
+        alg = sum(self.bytes_mode) / self.N
+        achieved = alg / (k_ms * 1e-3) / 1e9 if k_ms > 0 else 0.0
+        N = self.N
+        brk = {"remap_ms_per_sweep": tm["remap_ms"] / steps, "zero_ms_per_sweep": tm["zero_ms"] / steps,
+               "mttkrp_ms_per_sweep": tm["mttkrp_ms"] / steps, "fixup_ms_per_sweep": tm["fixup_ms"] / steps,
+               "remap_share": tm["remap_ms"] / total_k if total_k else None,
+               "remap_achieved_GBs": (N * self.remap_bytes_mode * steps) / (tm["remap_ms"] * 1e-3) / 1e9 if tm["remap_ms"] else None,
+               "mttkrp_only_GFLOPs": self.flops_per_sweep * steps / ((tm["mttkrp_ms"] + tm["zero_ms"] + tm["fixup_ms"]) * 1e-3) / 1e9
+               if tm["mttkrp_ms"] else None}
+        return k_ms, alg, achieved, brk
+
+    def close(self):
+        import torch
+        self.h.destroy()
+        self.fac = self.outs = None
+        torch.cuda.empty_cache()
+
+
+def extra_rows(P, W, args, dev, peak, skip_config):
+    """The other BASELINE.json configs and the rank sweep of configs[4], same procedure, fewer steps."""
+    rows = []
+    steps = max(5, min(args.steps, 10))
+    for c in range(len(W.CONFIGS)):
+        if c == skip_config:
+            continue
+        spec = W.CONFIGS[c]
+        ranks = list(spec.ranks) if len(spec.ranks) > 1 else [default_rank(spec)]
+        case = Case(P, W, spec, ranks[0], dev, max_rank=0)
+        for R in ranks:
+            case.set_rank(W, R)
+            for _ in range(3):
+                case.sweep()
+            ms, _, _ = case.timed_sweeps(steps)
+            k_ms, alg, achieved, brk = case.kernel_classes(steps)
+            rows.append({"workload": workload_name(spec, R), "value": case.flops_per_sweep / (ms / steps * 1e-3) / 1e9,
+                         "unit": UNIT, "ms_per_step": ms / steps, "steps": steps,
+                         "mttkrp_avg_launch_ms": k_ms, "mttkrp_algorithmic_GBs": achieved, "mttkrp_frac": achieved / peak,
+                         "remap_ms_per_sweep": brk["remap_ms_per_sweep"], "remap_share": brk["remap_share"],
+                         "create_s": case.create_s})
+        case.close()
+    return rows
+
+
 def run_ours(args):
     import torch
     import workloads as W
@@ -197,148 +374,99 @@ def run_ours(args):
     spec = W.CONFIGS[args.config]
     if args.nnz:
         spec = spec.scaled(args.nnz)
-    R = args.rank or spec.ranks[-1 if len(spec.ranks) == 1 else 2]
+    R = args.rank or default_rank(spec)
     N = len(spec.dims)
-    t_gen = time.perf_counter()
-    t = W.generate_tensor(spec, dev)
-    fac = W.generate_factors(spec, R, dev)
-    U = W.distinct_per_mode(t)
-    torch.cuda.synchronize()
-    t_gen = time.perf_counter() - t_gen
-    t_create = time.perf_counter()
-    h = P.Mttkrp(spec.dims, t.idx, t.vals, max_rank=0 if args.no_e2e else R)
-    torch.cuda.synchronize()
-    t_create = time.perf_counter() - t_create
-    checksums = t.checksums
-    nnz = t.nnz
-    sample_n = min(args.cpu_sample_nnz, nnz)
-    tensor_cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        tensor_cpu = (t.idx[:, :sample_n].cpu().numpy(), t.vals[:sample_n].cpu().numpy())
-    del t
-    torch.cuda.empty_cache()
-    info = h.info()
-    outs = [torch.empty((d, R), dtype=torch.float32, device=dev) for d in spec.dims]
+    want_cpu = rank == 0 and world == 1 and not args.no_cpu_baseline
+    case = Case(P, W, spec, R, dev, max_rank=0 if args.no_e2e else R, keep_coo=want_cpu)
+    info, nnz = case.info, case.nnz
+    warmup = max(args.warmup, 3)
 
-    # launches of OUR kernels per sweep: remap + zero-fill (if any empty row) + mttkrp + fix-up (if any split row)
-    launches_per_sweep = sum(2 + (1 if info["num_empty_rows"][d] else 0) + (1 if info["num_split_rows"][d] else 0)
-                             for d in range(N)) if nnz else sum(1 for d in range(N))
-    flops_per_sweep = float(nnz) * N * R * N
-    rec = info["record_bytes"]
-    bytes_mode = [nnz * rec + sum(U[m] for m in range(N) if m != d) * R * 4 + spec.dims[d] * R * 4 for d in range(N)]
-    remap_bytes_mode = nnz * (2 * rec + 4)
-
-    for _ in range(max(args.warmup, 3)):
-        h.mttkrp_sweep(fac, outs)
+    for _ in range(warmup):
+        case.sweep()
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
     time.sleep(0.25)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    w0 = time.time()
-    e0.record()
-    for _ in range(args.steps):
-        h.mttkrp_sweep(fac, outs)
-    e1.record()
-    barrier()
-    w1 = time.time()
-    ms_total = e0.elapsed_time(e1)
+    ms_total, w0, w1 = case.timed_sweeps(args.steps, barrier)
     clocks = sampler.stop(w0, w1)
     ms_total = replicas.max_over_ranks(ms_total, dev)
     ms_step = ms_total / args.steps
-    value = world * flops_per_sweep / (ms_step * 1e-3) / 1e9
+    value = world * case.flops_per_sweep / (ms_step * 1e-3) / 1e9
 
-    # per-kernel-class device time (CUDA events on the launching stream, inside the library)
-    h.timing_begin()
-    for _ in range(args.steps):
-        h.mttkrp_sweep(fac, outs)
-    tm = h.timing_end()
-    k_ms = tm["mttkrp_ms"] / max(1, tm["mttkrp_launches"])
-    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    if os.path.exists(peaks_path):
-        peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
-    else:
-        peak, peak_src = FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
-    alg_bytes_launch = sum(bytes_mode) / N
-    achieved = alg_bytes_launch / (k_ms * 1e-3) / 1e9 if k_ms > 0 else 0.0
-    traffic = l2_hit = l1_hit = None                   # ncu figures of that kernel, per launch (profiles/r1_traffic.csv)
-    tpath = os.path.join(ROOT, "profiles", "r1_traffic.csv")
-    if os.path.exists(tpath):
-        import csv
-        for row in csv.DictReader(open(tpath)):
-            if row["config"] == str(args.config) and row["kernel"] == "k_mttkrp" and not args.nnz and not args.rank:
-                traffic = float(row["dram_bytes_per_launch"])
-                l2_hit, l1_hit = float(row["l2_hit_pct"]), float(row["l1_hit_pct"])
-    total_k = tm["remap_ms"] + tm["zero_ms"] + tm["mttkrp_ms"] + tm["fixup_ms"]
+    peak, peak_src = hbm_peak()
+    k_ms, alg_bytes_launch, achieved, breakdown = case.kernel_classes(args.steps)
+    prof = ncu_traffic(args.config, R) if not args.nnz else None
     roofline = {"bound": "hbm", "kernel": "k_mttkrp", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
-                "l2_hit_pct_ncu": l2_hit, "l1_hit_pct_ncu": l1_hit,
-                "dram_GBs_ncu": (traffic / (k_ms * 1e-3) / 1e9) if (traffic and k_ms > 0) else None,
+                "frac": achieved / peak, "traffic": prof["traffic"] if prof else None, "peak_source": peak_src,
+                "traffic_source": (prof["source"] + " (ncu --set full capture of the committed build; a profile constant, "
+                                   "not measured by this run)") if prof else None,
+                "l2_hit_pct_ncu": prof["l2_hit_pct"] if prof else None, "l1_hit_pct_ncu": prof["l1_hit_pct"] if prof else None,
                 "frac_of_nominal_8TBs": achieved / 8000.0,
                 "algorithmic_bytes_per_launch": alg_bytes_launch, "avg_launch_ms": k_ms,
-                "per_mode_algorithmic_bytes": bytes_mode}
-    breakdown = {"remap_ms_per_sweep": tm["remap_ms"] / args.steps, "zero_ms_per_sweep": tm["zero_ms"] / args.steps,
-                 "mttkrp_ms_per_sweep": tm["mttkrp_ms"] / args.steps, "fixup_ms_per_sweep": tm["fixup_ms"] / args.steps,
-                 "remap_share": tm["remap_ms"] / total_k if total_k else None,
-                 "remap_achieved_GBs": (N * remap_bytes_mode * args.steps) / (tm["remap_ms"] * 1e-3) / 1e9 if tm["remap_ms"] else None,
-                 "mttkrp_only_GFLOPs": flops_per_sweep * args.steps / ((tm["mttkrp_ms"] + tm["zero_ms"] + tm["fixup_ms"]) * 1e-3) / 1e9
-                 if tm["mttkrp_ms"] else None}
+                "per_mode_algorithmic_bytes": case.bytes_mode,
+                "binding_limit": "L1 data pipe: one 128-byte wavefront per clock per SM, >= 1 per nonzero (DESIGN.md Sec. 6)"}
 
     # end to end through the host-buffer entry point (H2D of all factors + D2H of all Y_d every step)
     e2e = None
     if not args.no_e2e:
-        fac_host = [f.cpu().pin_memory() for f in fac]
+        fac_host = [f.cpu().pin_memory() for f in case.fac]
         out_host = [torch.empty((d, R), dtype=torch.float32).pin_memory() for d in spec.dims]
         for _ in range(2):
-            h.mttkrp_sweep_host(fac_host, out_host)
+            case.h.mttkrp_sweep_host(fac_host, out_host)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         e0.record()
         for _ in range(args.steps):
-            h.mttkrp_sweep_host(fac_host, out_host)
+            case.h.mttkrp_sweep_host(fac_host, out_host)
         e1.record()
         barrier()
-        ms_e2e = e0.elapsed_time(e1)
-        ms_e2e = replicas.max_over_ranks(ms_e2e, dev)
+        ms_e2e = replicas.max_over_ranks(e0.elapsed_time(e1), dev)
         io = sum(d * R * 4 for d in spec.dims)
-        e2e = {"value": world * flops_per_sweep / (ms_e2e / args.steps * 1e-3) / 1e9, "unit": UNIT,
+        e2e = {"value": world * case.flops_per_sweep / (ms_e2e / args.steps * 1e-3) / 1e9, "unit": UNIT,
                "h2d_bytes_per_step": io, "d2h_bytes_per_step": io, "ms_per_step": ms_e2e / args.steps,
                "api": "mttkrp_sweep_host (pinned host factors in, pinned host Y_d out)"}
+        del fac_host, out_host
 
     partition = None
     if args.partition_report:
         # Alg. 1 with one partition per SM: whole rows, longest first.  Equal-nnz shards are
         # balanced by construction (max/mean = 1); this shows what indivisible rows cost on the same tensor.
-        partition = {"kappa": 148, "max_over_mean": []}
+        kappa = torch.cuda.get_device_properties(dev).multi_processor_count
+        partition = {"kappa": kappa, "max_over_mean": []}
         for d in range(N):
-            _, loads = h.partition_rows(d, 148)
-            partition["max_over_mean"].append(round(float(loads.max()) / (float(loads.sum()) / 148), 3))
+            _, loads = case.h.partition_rows(d, kappa)
+            partition["max_over_mean"].append(round(float(loads.max()) / (float(loads.sum()) / kappa), 3))
         partition["note"] = "paper's Alg. 1 (whole rows, longest-first) on the same tensor; this library's equal-nnz shards: 1.0"
 
+    fac_np = [f.cpu().numpy() for f in case.fac] if want_cpu else None
+    coo = case.coo
+    details = {"replicas": world, "checksums": case.checksums, "distinct_per_mode": case.U,
+               "shard_nnz": info["shard_nnz"], "num_shards": info["num_shards"], "split_rows": info["num_split_rows"],
+               "empty_rows": info["num_empty_rows"], "key_order": info["key_order"],
+               "remap_blocked": info["remap_blocked"], "remap_avg_run": [round(x, 1) for x in info["remap_avg_run"]],
+               "bytes_held": info["bytes_held"], "bytes_paper_format": info["bytes_paper_format"],
+               "create_s": case.create_s, "generate_s": case.generate_s}
+    launches = case.launches_per_sweep * args.steps
+    case.close()
+
+    extra = None
+    if rank == 0 and world == 1 and not args.no_extra and not args.nnz:
+        extra = extra_rows(P, W, args, dev, peak, args.config)
+
     cpu_baseline = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cpu_baseline, _, _ = time_oracle_sample(spec, R, sample_n, tensor_cpu)
+    if want_cpu:
+        cpu_baseline = cpu_baseline_leg(spec, R, coo[0], coo[1], fac_np, args.cpu_sample_nnz)
 
     if rank == 0:
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warmup,
                 "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
-                "data": "synthetic",
-                "config": {"workload": workload_name(spec, R), "nmodes": N, "nnz": nnz, "R": R,
-                           "step": f"one sweep = {N} remaps + {N} MTTKRPs", "l2": "inputs larger than L2 (2 tensor copies of "
-                           f"{nnz * rec / 1e6:.0f} MB each alternate; L2 is 126 MB)", "replicas": world,
-                           "checksums": checksums, "distinct_per_mode": U, "shard_nnz": info["shard_nnz"],
-                           "num_shards": info["num_shards"], "split_rows": info["num_split_rows"],
-                           "empty_rows": info["num_empty_rows"], "key_order": info["key_order"],
-                           "remap_blocked": info["remap_blocked"],
-                           "remap_avg_run": [round(x, 1) for x in info["remap_avg_run"]],
-                           "bytes_held": info["bytes_held"], "bytes_paper_format": info["bytes_paper_format"],
-                           "create_s": t_create, "generate_s": t_gen},
-                "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_sweep * args.steps,
-                "roofline": roofline, "breakdown": breakdown, "cpu_baseline": cpu_baseline, "partition": partition,
+                "data": "synthetic", "config": config_block(spec, R), "details": details,
+                "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
+                "roofline": roofline, "breakdown": breakdown, "cpu_baseline": cpu_baseline, "extra": extra,
+                "partition": partition,
                 "paper_context": "geomean speedups 1.5x / 2.0x / 21.7x over BLCO / MM-CSF / ParTI-GPU on RTX 3090 "
                                  "(PAPER.md:414); no absolute numbers published"}
         print(json.dumps(line), flush=True)
-    h.destroy()
     replicas.finalize()
 
 

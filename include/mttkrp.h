@@ -25,6 +25,13 @@
  *   - Indices are 0-based.  Duplicate coordinates are legal and add.  nnz == 0 is legal.
  *   - There is no CPU fallback: without a CUDA device every compute call returns MTTKRP_ECUDA.
  *   - A handle is not thread-safe; distinct handles are independent.
+ *   - Calls on one handle execute in call order even when they are given different streams: the handle
+ *     remembers the stream of its last call and makes a call on another stream wait (cudaStreamWaitEvent) for
+ *     the work launched before it.  The caller still orders its own use of `out` and of the factor buffers.
+ *   - Process environment variables read by mttkrp_workspace_bytes / mttkrp_create (test and experiment knobs;
+ *     unset = the library decides): MTTKRP_KEY_ORDER = revcyclic|desc|asc|cyclic (anything else: EINVAL),
+ *     MTTKRP_PACK = 0|1, MTTKRP_REMAP_BLOCKED = 0|1, MTTKRP_REMAP_BLOCK_LOG2 (clamped to [10,26]),
+ *     MTTKRP_FORCE_DEEP = 0|1 (kernel variant).  They must not change between the size query and create.
  */
 #ifndef MTTKRP_B200_H
 #define MTTKRP_B200_H
@@ -55,7 +62,8 @@ typedef struct {
     int32_t cur_layout;                  /* mode whose order the resident tensor copy is in (0 after create) */
     int64_t nnz;
     int64_t dims[MTTKRP_MAX_MODES];
-    int32_t record_bytes;                /* bytes per nonzero in the device format: 4*(nmodes+1) */
+    int32_t record_bytes;                /* bytes per nonzero in the device format: 16 for nmodes == 3 and for the
+                                            bit-packed records of nmodes >= 4, else 4*(nmodes+1) */
     int32_t shard_nnz;                   /* nonzeros per thread-block shard */
     int64_t num_shards;                  /* ceil(nnz / shard_nnz); same for every mode */
     int64_t num_split_rows[MTTKRP_MAX_MODES];  /* output rows whose nonzeros span more than one shard */
@@ -105,8 +113,9 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
  *            factors[d] is not read and may be NULL.
  *   out:     device fp32 [dims[d]][R] row-major; fully overwritten (rows without nonzeros get 0).
  *            Must not alias a factor that is read.
- *   Any d in any order.  If the resident layout is not d the tensor is first remapped
- *   (cur -> cur+1 -> ... -> d, one gather pass per step; the cyclic order of Alg. 5 costs one).
+ *   Any d in any order.  If the resident layout is not d the tensor is first remapped: one gather pass
+ *   (the cyclic order of Alg. 5, d == cur+1, uses the stored walk; any other d first composes the stored
+ *   position maps into one direct map cur -> d, cached for the next identical jump).
  */
 mttkrp_status_t mttkrp_mode(mttkrp_handle_t h, int d, const float* const* factors, int R,
                             float* out, void* cuda_stream);
@@ -130,7 +139,8 @@ mttkrp_status_t mttkrp_remap_to(mttkrp_handle_t h, int d, void* cuda_stream);
 mttkrp_status_t mttkrp_sweep_host(mttkrp_handle_t h, const float* const* factors, int R,
                                   float* const* outs, void* cuda_stream);
 
-/* Frees the host object.  Touches no device memory; the workspace is the caller's again. */
+/* Frees the host object.  Blocks until the work this handle launched has finished (the workspace is the
+ * caller's again on return); touches no device memory itself. */
 mttkrp_status_t mttkrp_destroy(mttkrp_handle_t h);
 
 /* Thread-local message of the last failing call ("" if none). */

@@ -3,7 +3,7 @@
 Textbook CPD-ALS (the paper names it, and gives no further detail) on top of the oracle's
 MTTKRP: for d = 0..N-1: M = MTTKRP_d; G = Hadamard_{m != d} A_m^T A_m; A_d = M G^{-1}; normalise columns.
 fit = 1 - ||X - X^|| / ||X|| with <X, X^> = sum_r lam_r sum_i M[i,r] A_d[i,r], ||X^||^2 = lam^T (Hadamard_m
-A_m^T A_m) lam.  Pinned in tests/test_oracle_pins.py: an exactly rank-R tensor is recovered (fit -> 1), the fit
+A_m^T A_m) lam.  Pinned in tests/test_cpd.py: an exactly rank-R tensor is recovered (fit -> 1), the fit
 never decreases, and the fit formula equals the explicit dense residual.
 """
 from __future__ import annotations

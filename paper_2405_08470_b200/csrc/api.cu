@@ -45,8 +45,43 @@ static int ceil_log2(int64_t x) {
     return b;
 }
 
+// Layout state machine (Alg. 5's swap).  d == cur: nothing.  d == cur+1:
+// the stored walk (the paper's only case).  Any other d: the stored gather maps of the layouts in
+// between are composed into ONE direct map cur -> d (4-byte gathers), cached for the next identical jump, and the
+// records move once.  Layouts are absolute orders (remap ids are positions), so the result does
+// not depend on the path.
 static mttkrp_status_t ensure_layout(mttkrp_handle_s* h, int d, cudaStream_t st) {
-    while (h->cur != d) MK_TRY(launch_remap(h, h->cur, st));
+    if (h->cur == d) return MTTKRP_OK;
+    const int N = h->N, from = h->cur;
+    const int steps = ((d - from) % N + N) % N;
+    if (steps == 1 || h->nnz == 0) return launch_remap(h, from, d, nullptr, st);
+    if (!(h->jump_map && h->jump_from == from && h->jump_to == d)) {
+        // acc_s[j] = position in layout `from` of the element at position j of layout from+s
+        const uint32_t* acc = h->mode[from].next;
+        for (int s = 1; s < steps; ++s) {
+            uint32_t* outb = h->jump[(s - 1) & 1];
+            TimedLaunch tl(h->timing, kClsRemap, st);
+            MK_TRY(launch_perm_step(h->mode[(from + s) % N].next, acc, outb, h->nnz, st));
+            acc = outb;
+        }
+        h->jump_map = acc;
+        h->jump_from = from;
+        h->jump_to = d;
+    }
+    return launch_remap(h, from, d, h->jump_map, st);
+}
+
+// Calls on one handle share the two tensor copies and the carry buffer, so they must execute in call order.
+// The handle remembers the stream of its last call and an event recorded after it; a call that arrives on a
+// different stream first makes that stream wait on the event.
+static mttkrp_status_t order_begin(mttkrp_handle_s* h, cudaStream_t st) {
+    if (h->launched && st != h->last_stream) MK_CUDA(cudaStreamWaitEvent(st, h->ev_order, 0));
+    return MTTKRP_OK;
+}
+static mttkrp_status_t order_end(mttkrp_handle_s* h, cudaStream_t st) {
+    MK_CUDA(cudaEventRecord(h->ev_order, st));
+    h->last_stream = st;
+    h->launched = 1;
     return MTTKRP_OK;
 }
 
@@ -71,9 +106,9 @@ mttkrp_status_t mttkrp_workspace_bytes(int nmodes, const int64_t* dims, int64_t 
     MK_TRY(check_shape(nmodes, dims, nnz));
     if (max_rank != 0 && !valid_rank(max_rank)) { set_error("max_rank %d not in {0,8,16,32,64}", max_rank); return MTTKRP_EUNSUPPORTED; }
     LayoutPlan lp;
-    plan_layouts(nmodes, dims, nnz, &lp);
+    MK_TRY(plan_layouts(nmodes, dims, nnz, &lp));
     WorkspacePlan p;
-    MK_TRY(plan_workspace(nmodes, dims, nnz, max_rank, lp.rec_words, &p));
+    MK_TRY(plan_workspace(nmodes, dims, nnz, max_rank, lp.rec_words, device_sm_count(), &p));
     *bytes = p.total;
     return MTTKRP_OK;
 }
@@ -90,9 +125,10 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
     if (reinterpret_cast<uintptr_t>(workspace) & 255u) { set_error("workspace must be 256-byte aligned"); return MTTKRP_EWORKSPACE; }
     if (nnz > 0 && (!aligned16(idx) || !aligned16(vals))) { set_error("idx/vals must be 16-byte aligned"); return MTTKRP_EINVAL; }
     LayoutPlan lp;
-    plan_layouts(nmodes, dims, nnz, &lp);
+    MK_TRY(plan_layouts(nmodes, dims, nnz, &lp));
     WorkspacePlan p;
-    MK_TRY(plan_workspace(nmodes, dims, nnz, max_rank, lp.rec_words, &p));
+    const int num_sms = device_sm_count();
+    MK_TRY(plan_workspace(nmodes, dims, nnz, max_rank, lp.rec_words, num_sms, &p));
     if (workspace_bytes < p.total) {
         set_error("workspace %zu bytes < required %zu", workspace_bytes, p.total);
         return MTTKRP_EWORKSPACE;
@@ -118,6 +154,20 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
     h->cur = 0;
     h->max_rank = max_rank;
     h->device = dev;
+    h->num_sms = num_sms;
+    {
+        const char* env = getenv("MTTKRP_FORCE_DEEP");               // tests: 0 / 1 pins the kernel variant
+        h->force_deep = env ? (env[0] == '1' ? 1 : 0) : -1;
+    }
+    h->jump[0] = reinterpret_cast<uint32_t*>(ws + p.jump[0]);
+    h->jump[1] = reinterpret_cast<uint32_t*>(ws + p.jump[1]);
+    h->jump_map = nullptr;
+    h->jump_from = h->jump_to = -1;
+    if (cudaEventCreateWithFlags(&h->ev_order, cudaEventDisableTiming) != cudaSuccess) {
+        set_error("cudaEventCreate failed");
+        delete h;
+        return MTTKRP_ECUDA;
+    }
     h->timing = new (std::nothrow) Timing();
     for (int d = 0; d < nmodes; ++d) {
         ModeMeta& mm = h->mode[d];
@@ -137,7 +187,8 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
     }
     h->bytes_held = (int64_t)(p.persistent_end + (size_t)lp.rec_words * 4 * (size_t)(p.num_shards * p.shard_nnz));
     mttkrp_status_t s = build_format(h, p, ws, idx, vals, static_cast<cudaStream_t>(cuda_stream));
-    if (s != MTTKRP_OK) { delete h->timing; delete h; return s; }
+    if (s != MTTKRP_OK) { cudaEventDestroy(h->ev_order); delete h->timing; delete h; return s; }
+    order_end(h, static_cast<cudaStream_t>(cuda_stream));
     *out = h;
     return MTTKRP_OK;
 }
@@ -160,7 +211,10 @@ static mttkrp_status_t check_mode_args(mttkrp_handle_t h, int d, const float* co
 mttkrp_status_t mttkrp_mode(mttkrp_handle_t h, int d, const float* const* factors, int R, float* out, void* cuda_stream) {
     MK_TRY(check_mode_args(h, d, factors, R, out));
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    return run_mode(h, d, factors, R, out, st);
+    MK_TRY(order_begin(h, st));
+    const mttkrp_status_t s = run_mode(h, d, factors, R, out, st);
+    MK_TRY(order_end(h, st));
+    return s;
 }
 
 mttkrp_status_t mttkrp_sweep(mttkrp_handle_t h, const float* const* factors, int R, float* const* outs, void* cuda_stream) {
@@ -174,7 +228,11 @@ mttkrp_status_t mttkrp_sweep(mttkrp_handle_t h, const float* const* factors, int
 mttkrp_status_t mttkrp_remap_to(mttkrp_handle_t h, int d, void* cuda_stream) {
     if (!h) { set_error("handle is NULL"); return MTTKRP_EINVAL; }
     if (d < 0 || d >= h->N) { set_error("mode %d outside [0,%d)", d, h->N); return MTTKRP_EINVAL; }
-    return ensure_layout(h, d, static_cast<cudaStream_t>(cuda_stream));
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    MK_TRY(order_begin(h, st));
+    const mttkrp_status_t s = ensure_layout(h, d, st);
+    MK_TRY(order_end(h, st));
+    return s;
 }
 
 mttkrp_status_t mttkrp_sweep_host(mttkrp_handle_t h, const float* const* factors, int R, float* const* outs,
@@ -199,6 +257,7 @@ mttkrp_status_t mttkrp_sweep_host(mttkrp_handle_t h, const float* const* factors
     // Copies overlap the kernels: factors go in on one stream (A_0, which mode 0 does not read, last), every
     // Y_d goes out on another while the next mode runs; the caller's stream carries the kernels.
     const float* dfac[kMaxModes];
+    MK_TRY(order_begin(h, st));
     MK_CUDA(cudaEventRecord(h->ev_sync, st));
     MK_CUDA(cudaStreamWaitEvent(h->s_in, h->ev_sync, 0));
     for (int i = 0; i < h->N; ++i) {
@@ -218,6 +277,7 @@ mttkrp_status_t mttkrp_sweep_host(mttkrp_handle_t h, const float* const* factors
         MK_CUDA(cudaStreamWaitEvent(h->s_out, h->ev_done[d], 0));
         MK_CUDA(cudaMemcpyAsync(outs[d], h->stage_out[d], (size_t)h->dims[d] * R * 4, cudaMemcpyDeviceToHost, h->s_out));
     }
+    MK_TRY(order_end(h, st));
     MK_CUDA(cudaStreamSynchronize(st));
     MK_CUDA(cudaStreamSynchronize(h->s_out));
     return MTTKRP_OK;
@@ -225,6 +285,9 @@ mttkrp_status_t mttkrp_sweep_host(mttkrp_handle_t h, const float* const* factors
 
 mttkrp_status_t mttkrp_destroy(mttkrp_handle_t h) {
     if (!h) { set_error("handle is NULL"); return MTTKRP_EINVAL; }
+    // The workspace goes back to the caller: wait until the handle's last launched work has finished with it.
+    if (h->launched) cudaEventSynchronize(h->ev_order);
+    cudaEventDestroy(h->ev_order);
     if (h->timing) {
         for (auto& e : h->timing->ev) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
         delete h->timing;
@@ -301,7 +364,8 @@ mttkrp_status_t mttkrp_get_perm(mttkrp_handle_t h, int d, uint32_t* perm_dev, ui
     if (h->nnz == 0) return MTTKRP_OK;
     if (!perm_dev || (d > 0 && !scratch_dev)) { set_error("perm/scratch is NULL"); return MTTKRP_EINVAL; }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    // perm_{j+1}[next_j[k]] = perm_j[k]; choose the start buffer so that step d lands in perm_dev.
+    MK_TRY(order_begin(h, st));
+    // perm_{j+1}[k] = perm_j[next_j[k]]; choose the start buffer so that step d lands in perm_dev.
     uint32_t* a = (d % 2 == 0) ? perm_dev : scratch_dev;
     uint32_t* b = (d % 2 == 0) ? scratch_dev : perm_dev;
     MK_CUDA(cudaMemcpyAsync(a, h->perm0, (size_t)h->nnz * 4, cudaMemcpyDeviceToDevice, st));
@@ -309,14 +373,17 @@ mttkrp_status_t mttkrp_get_perm(mttkrp_handle_t h, int d, uint32_t* perm_dev, ui
         MK_TRY(launch_perm_step(h->mode[j].next, a, b, h->nnz, st));
         uint32_t* t = a; a = b; b = t;
     }
-    return MTTKRP_OK;
+    return order_end(h, st);
 }
 
 mttkrp_status_t mttkrp_export_coo(mttkrp_handle_t h, int32_t* idx_dev, float* vals_dev, void* cuda_stream) {
     if (!h) { set_error("handle is NULL"); return MTTKRP_EINVAL; }
     if (h->nnz == 0) return MTTKRP_OK;
     if (!idx_dev || !vals_dev) { set_error("idx/vals is NULL"); return MTTKRP_EINVAL; }
-    return launch_export(h, idx_dev, vals_dev, static_cast<cudaStream_t>(cuda_stream));
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    MK_TRY(order_begin(h, st));
+    MK_TRY(launch_export(h, idx_dev, vals_dev, st));
+    return order_end(h, st);
 }
 
 mttkrp_status_t mttkrp_partition_rows(mttkrp_handle_t h, int d, int kappa, int32_t* deg_dev, int32_t* part_of_row,
@@ -326,8 +393,11 @@ mttkrp_status_t mttkrp_partition_rows(mttkrp_handle_t h, int d, int kappa, int32
     if (kappa < 1) { set_error("kappa %d < 1", kappa); return MTTKRP_EINVAL; }
     if (!deg_dev || !loads) { set_error("deg_dev/loads is NULL"); return MTTKRP_EINVAL; }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    MK_TRY(order_begin(h, st));
     MK_TRY(launch_row_degrees(h, d, deg_dev, st));
+    MK_TRY(order_end(h, st));
     const int64_t rows = h->dims[d];
+    try {                                                      // std::vector / stable_sort may throw: nothing crosses the C ABI
     std::vector<int32_t> deg((size_t)rows);
     MK_CUDA(cudaMemcpyAsync(deg.data(), deg_dev, sizeof(int32_t) * (size_t)rows, cudaMemcpyDeviceToHost, st));
     MK_CUDA(cudaStreamSynchronize(st));
@@ -346,6 +416,10 @@ mttkrp_status_t mttkrp_partition_rows(mttkrp_handle_t h, int d, int kappa, int32
         loads[b.second] = b.first;
         if (part_of_row) part_of_row[v] = b.second;
         heap.push(b);
+    }
+    } catch (...) {
+        set_error("mttkrp_partition_rows: out of host memory");
+        return MTTKRP_EINVAL;
     }
     return MTTKRP_OK;
 }

@@ -23,17 +23,28 @@ constexpr int kScanThreads = 256;
 constexpr int kScanItems = 8;
 constexpr int kScanTile = kScanThreads * kScanItems;
 
-static int choose_shard_nnz(int64_t nnz) {
-    // Aim for >= 8 shards per SM on 148 SMs; power of two in [kMinShardNnz, kMaxShardNnz].
+int device_sm_count() {
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) {
+        (void)cudaGetLastError();
+        return 148;                                   // B200; only reached without a device (size queries on a CPU box)
+    }
+    return sms;
+}
+
+static int choose_shard_nnz(int64_t nnz, int num_sms) {
+    // Aim for >= 8 shards per SM; power of two in [kMinShardNnz, kMaxShardNnz].
     int s = kMaxShardNnz;
-    while (s > kMinShardNnz && nnz / s < 148 * 8) s >>= 1;
+    while (s > kMinShardNnz && nnz / s < (int64_t)num_sms * 8) s >>= 1;
     return s;
 }
 
-mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_rank, int rec_words, WorkspacePlan* p) {
+mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_rank, int rec_words, int num_sms,
+                               WorkspacePlan* p) {
     memset(p, 0, sizeof(*p));
     const size_t n = (size_t)nnz;
-    p->shard_nnz = choose_shard_nnz(nnz);
+    p->shard_nnz = choose_shard_nnz(nnz, num_sms);
     p->num_shards = (nnz + p->shard_nnz - 1) / p->shard_nnz;
     // both tensor copies are padded to a whole number of shards (zero-valued copies of the last nonzero)
     const size_t rec_bytes = (size_t)rec_words * 4 * (size_t)(p->num_shards * p->shard_nnz);
@@ -44,6 +55,9 @@ mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_
     for (int d = 0; d < N; ++d) { p->osrc[d] = off; off = align_up(off + 4 * n); }
     for (int d = 0; d < N; ++d) { p->lflags[d] = off; off = align_up(off + (size_t)(p->num_shards * p->shard_nnz)); }
     p->perm0 = off; off = align_up(off + 4 * n);
+    // composed maps for out-of-order calls: a jump of k layouts composes k-1 times (ping-pong when k > 2)
+    p->jump[0] = off; if (N >= 3) off = align_up(off + 4 * n);
+    p->jump[1] = off; if (N >= 4) off = align_up(off + 4 * n);
     for (int d = 0; d < N; ++d) { p->empty[d] = off; off = align_up(off + 4 * (size_t)dims[d]); }
     for (int d = 0; d < N; ++d) { p->chains[d] = off; off = align_up(off + 12 * (size_t)p->num_shards); }
     p->carry = off; off = align_up(off + (size_t)2 * p->num_shards * kMaxRank * 4);
@@ -400,6 +414,10 @@ static int ceil_log2_i64(int64_t x) {
     return b;
 }
 
+static bool known_key_order(const char* s) {
+    return !strcmp(s, "revcyclic") || !strcmp(s, "desc") || !strcmp(s, "asc") || !strcmp(s, "cyclic");
+}
+
 void choose_key_order(int N, const int64_t* dims, int d, const char* env, int* order) {
     // Default: order[d] = (d, d-1, d-2, ..., d-N+1) (mod N).  The layout of mode d+1 is then
     // (last key of layout d, then the keys of layout d in their order), so inside one output row of
@@ -425,13 +443,17 @@ void choose_key_order(int N, const int64_t* dims, int d, const char* env, int* o
     for (int j = 0; j < n; ++j) order[j + 1] = rest[j];
 }
 
-void plan_layouts(int N, const int64_t* dims, int64_t nnz, LayoutPlan* lp) {
+mttkrp_status_t plan_layouts(int N, const int64_t* dims, int64_t nnz, LayoutPlan* lp) {
     // Key order of the layouts (reading 4).  The default makes every remap a stable partition
     // by one key, which the blocked remap turns into L2-resident gathers; that pays when the nonzeros a
     // source block sends to one output row form runs of several records.  The expected run for mode d
     // is nnz / (dims[d] * number of blocks); when most modes are too large for that, the size-ordered
     // tuple (one remap of the cycle moves whole fibers) is the better choice.
     const char* order_env = getenv("MTTKRP_KEY_ORDER");
+    if (order_env && !known_key_order(order_env)) {
+        set_error("MTTKRP_KEY_ORDER=%s is not one of revcyclic, desc, asc, cyclic", order_env);
+        return MTTKRP_EINVAL;
+    }
     if (!order_env) {
         const double nblk = (double)((nnz >> 20) > 0 ? (nnz >> 20) : 1);
         int good = 0;
@@ -455,6 +477,7 @@ void plan_layouts(int N, const int64_t* dims, int64_t nnz, LayoutPlan* lp) {
     }
     lp->packed = packed ? 1 : 0;
     lp->rec_words = packed ? 4 : N + 1;
+    return MTTKRP_OK;
 }
 
 mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char* ws, const int32_t* idx,
@@ -593,6 +616,7 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
             const char* env = getenv("MTTKRP_REMAP_BLOCK_LOG2");
             if (env) block_log2 = atoi(env);
             if (block_log2 < 10) block_log2 = 10;
+            if (block_log2 > 26) block_log2 = 26;                     // 2^26 records = 1 GB windows: far beyond any L2
             while ((nnz >> block_log2) > 255) ++block_log2;            // at most 256 blocks (one radix digit)
         }
         for (int d = 0; d < N; ++d) {

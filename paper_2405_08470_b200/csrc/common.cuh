@@ -134,12 +134,20 @@ struct mttkrp_handle_s {
     mk::ModeMeta mode[mk::kMaxModes];
     float* carry;             // [2*num_shards][kMaxRank] partial rows of split rows
     int cur;
+    uint32_t* jump[2];        // [nnz] each: composed gather maps for out-of-order calls (api.cu ensure_layout)
+    const uint32_t* jump_map; // the cached composed map (points into jump[]) and the transition it serves
+    int jump_from, jump_to;
     int max_rank;
     float* stage_fac[mk::kMaxModes];
     float* stage_out[mk::kMaxModes];
     int64_t bytes_held;
     int64_t remaps_done;
     int device;
+    int num_sms;              // SM count of `device` (grid sizing)
+    int force_deep;           // MTTKRP_FORCE_DEEP at create: -1 = by factor size (default), 0 / 1 = never / always
+    cudaStream_t last_stream; // stream of the last call that launched work for this handle
+    cudaEvent_t ev_order;     // recorded on last_stream after every such call: a call on another stream waits on it
+    int launched;             // ev_order has been recorded at least once
     mk::Timing* timing;       // owned; per-kernel event pairs while mttkrp_timing_begin is active
     cudaStream_t s_in, s_out; // copy streams of mttkrp_sweep_host (created on first use)
     cudaEvent_t ev_in[mk::kMaxModes], ev_done[mk::kMaxModes], ev_sync;
@@ -150,7 +158,7 @@ namespace mk {
 
 // ---- build.cu -------------------------------------------------------------------------------
 struct WorkspacePlan {
-    size_t rec_a, rec_b, perm0, carry;
+    size_t rec_a, rec_b, perm0, carry, jump[2];
     size_t next[kMaxModes], empty[kMaxModes], chains[kMaxModes], ord[kMaxModes], osrc[kMaxModes], lflags[kMaxModes];
     size_t stage_fac[kMaxModes], stage_out[kMaxModes];
     size_t persistent_end;
@@ -166,13 +174,14 @@ struct LayoutPlan {
     int packed;
     int rec_words;
 };
-void plan_layouts(int N, const int64_t* dims, int64_t nnz, LayoutPlan* lp);
-mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_rank, int rec_words, WorkspacePlan* p);
+mttkrp_status_t plan_layouts(int N, const int64_t* dims, int64_t nnz, LayoutPlan* lp);   // EINVAL: bad MTTKRP_* override
+mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_rank, int rec_words, int num_sms, WorkspacePlan* p);
+int device_sm_count();       // SM count of the current device (148 when no device can be queried)
 mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char* ws,
                              const int32_t* idx, const float* vals, cudaStream_t st);
 
 // ---- remap.cu -------------------------------------------------------------------------------
-mttkrp_status_t launch_remap(mttkrp_handle_s* h, int from, cudaStream_t st);   // from -> (from+1)%N, swaps copies
+mttkrp_status_t launch_remap(mttkrp_handle_s* h, int from, int to, const uint32_t* jump, cudaStream_t st);   // swaps copies
 mttkrp_status_t launch_export(const mttkrp_handle_s* h, int32_t* idx, float* vals, cudaStream_t st);
 mttkrp_status_t launch_row_degrees(const mttkrp_handle_s* h, int d, int32_t* deg_dev, cudaStream_t st);
 mttkrp_status_t launch_perm_step(const uint32_t* map, const uint32_t* in, uint32_t* out, int64_t nnz, cudaStream_t st);

@@ -483,7 +483,7 @@ static mttkrp_status_t launch_nr(mttkrp_handle_s* h, int d, const float* const* 
     if (mm.n_empty > 0) {
         const int64_t groups = mm.n_empty;
         const int64_t threads = groups * (R / 4);
-        const unsigned grid = (unsigned)std::min<int64_t>((threads + 255) / 256, 148 * 16);
+        const unsigned grid = (unsigned)std::min<int64_t>((threads + 255) / 256, (int64_t)h->num_sms * 16);
         TimedLaunch tl(h->timing, kClsZero, st);
         k_zero_rows<R><<<grid, 256, 0, st>>>(mm.empty_rows, mm.n_empty, out);
     }
@@ -500,7 +500,7 @@ static mttkrp_status_t launch_nr(mttkrp_handle_s* h, int d, const float* const* 
         // variant with the deeper look-ahead (measured on configs[2]: 2.96 vs 3.19 ms per mode).
         int64_t fac_bytes = 0;
         for (int l = 1; l < N; ++l) fac_bytes += h->dims[mm.order[l]] * (int64_t)R * 4;
-        const bool deep = N <= 3 && fac_bytes > (96ll << 20);
+        const bool deep = N <= 3 && (h->force_deep >= 0 ? h->force_deep == 1 : fac_bytes > (96ll << 20));
         for (int l = 0; l < N; ++l) { a.kmask[l] = 0xffffffffu; a.koff[l] = 0; }
         if (h->packed)
             for (int l = 0; l < N; ++l) { a.kmask[l] = pk_mask(mm.pk.bits[l]); a.koff[l] = mm.pk.off[l]; }

@@ -135,13 +135,17 @@ __global__ void __launch_bounds__(256) k_remap_pk(const uint4* __restrict__ in, 
     }
 }
 
+// The walk of one remap pass: `map[j]` = source position of destination position j; blocked walks also carry
+// `ord` / `osrc` (see k_remap3).
+struct Walk { const uint32_t* map; const uint32_t* ord; const uint32_t* osrc; int blocked; };
+
 template <int N>
-static void launch_remap_n(mttkrp_handle_s* h, int from, int to, unsigned grid, int64_t nnz_pad, const FieldMap& fm, cudaStream_t st) {
+static void launch_remap_n(mttkrp_handle_s* h, int from, int to, const Walk& w, unsigned grid, int64_t nnz_pad, const FieldMap& fm, cudaStream_t st) {
     const ModeMeta& mf = h->mode[from];
     const uint8_t* dflags = h->mode[to].lflags;
     if constexpr (N == 3) {
-        if (mf.blocked) k_remap3<true><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, mf.next, mf.ord, mf.osrc, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, fm);
-        else k_remap3<false><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, mf.next, mf.ord, mf.osrc, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, fm);
+        if (w.blocked) k_remap3<true><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, w.map, w.ord, w.osrc, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, fm);
+        else k_remap3<false><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, w.map, w.ord, w.osrc, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, fm);
     } else {
         if constexpr (N >= 4) {
             if (h->packed) {
@@ -153,35 +157,42 @@ static void launch_remap_n(mttkrp_handle_s* h, int from, int to, unsigned grid, 
                     rp.smask[l] = pk_mask(mf.pk.bits[sl]);
                 }
                 const PackDesc dd = h->mode[to].pk;
-                if (mf.blocked) k_remap_pk<N, true><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, mf.next, mf.ord, mf.osrc, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, rp, dd);
-                else k_remap_pk<N, false><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, mf.next, mf.ord, mf.osrc, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, rp, dd);
+                if (w.blocked) k_remap_pk<N, true><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, w.map, w.ord, w.osrc, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, rp, dd);
+                else k_remap_pk<N, false><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, w.map, w.ord, w.osrc, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, rp, dd);
                 return;
             }
         }
-        if (mf.blocked) k_remap<N, true><<<grid, 256, 0, st>>>(h->rec_cur, mf.next, mf.ord, dflags, h->rec_alt, h->nnz, nnz_pad, fm);
-        else k_remap<N, false><<<grid, 256, 0, st>>>(h->rec_cur, mf.next, mf.ord, dflags, h->rec_alt, h->nnz, nnz_pad, fm);
+        if (w.blocked) k_remap<N, true><<<grid, 256, 0, st>>>(h->rec_cur, w.map, w.ord, dflags, h->rec_alt, h->nnz, nnz_pad, fm);
+        else k_remap<N, false><<<grid, 256, 0, st>>>(h->rec_cur, w.map, w.ord, dflags, h->rec_alt, h->nnz, nnz_pad, fm);
     }
 }
 
-mttkrp_status_t launch_remap(mttkrp_handle_s* h, int from, cudaStream_t st) {
+// One gather pass from layout `from` into layout `to`, then swap(T_in, T_out).  jump == nullptr: the stored
+// walk of the transition from -> (from+1)%N (the paper's only case).  Otherwise `jump[j]` is the
+// position in layout `from` of the element at position j of layout `to` (composed by api.cu for out-of-order
+// calls): plain walk in destination order.
+mttkrp_status_t launch_remap(mttkrp_handle_s* h, int from, int to, const uint32_t* jump, cudaStream_t st) {
     const int N = h->N;
-    const int to = (from + 1) % N;
     if (h->nnz > 0) {
+        const ModeMeta& mf = h->mode[from];
+        Walk w;
+        if (jump) { w.map = jump; w.ord = nullptr; w.osrc = nullptr; w.blocked = 0; }
+        else { w.map = mf.next; w.ord = mf.ord; w.osrc = mf.osrc; w.blocked = mf.blocked; }
         FieldMap fm;
         for (int l = 0; l < kMaxModes; ++l) fm.src[l] = 0;
         for (int l = 0; l < N; ++l) fm.src[l] = h->mode[from].pos[h->mode[to].order[l]];
         const int64_t nnz_pad = h->num_shards * (int64_t)h->shard_nnz;
-        const int per_block = 256 * (h->mode[from].blocked ? remap_per_thread<true>() : remap_per_thread<false>());
+        const int per_block = 256 * (w.blocked ? remap_per_thread<true>() : remap_per_thread<false>());
         const unsigned grid = (unsigned)((nnz_pad + per_block - 1) / per_block);
         TimedLaunch tl(h->timing, kClsRemap, st);
         switch (N) {
-            case 2: launch_remap_n<2>(h, from, to, grid, nnz_pad, fm, st); break;
-            case 3: launch_remap_n<3>(h, from, to, grid, nnz_pad, fm, st); break;
-            case 4: launch_remap_n<4>(h, from, to, grid, nnz_pad, fm, st); break;
-            case 5: launch_remap_n<5>(h, from, to, grid, nnz_pad, fm, st); break;
-            case 6: launch_remap_n<6>(h, from, to, grid, nnz_pad, fm, st); break;
-            case 7: launch_remap_n<7>(h, from, to, grid, nnz_pad, fm, st); break;
-            case 8: launch_remap_n<8>(h, from, to, grid, nnz_pad, fm, st); break;
+            case 2: launch_remap_n<2>(h, from, to, w, grid, nnz_pad, fm, st); break;
+            case 3: launch_remap_n<3>(h, from, to, w, grid, nnz_pad, fm, st); break;
+            case 4: launch_remap_n<4>(h, from, to, w, grid, nnz_pad, fm, st); break;
+            case 5: launch_remap_n<5>(h, from, to, w, grid, nnz_pad, fm, st); break;
+            case 6: launch_remap_n<6>(h, from, to, w, grid, nnz_pad, fm, st); break;
+            case 7: launch_remap_n<7>(h, from, to, w, grid, nnz_pad, fm, st); break;
+            case 8: launch_remap_n<8>(h, from, to, w, grid, nnz_pad, fm, st); break;
             default: set_error("remap: unsupported nmodes %d", N); return MTTKRP_EUNSUPPORTED;
         }
         MK_CUDA(cudaGetLastError());

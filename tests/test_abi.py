@@ -65,6 +65,17 @@ def test_bad_shapes_are_rejected(lib, dims, nnz, rank, status):
     assert str(e.value)
 
 
+def test_environment_overrides_are_validated(lib, monkeypatch):
+    import paper_2405_08470_b200 as P
+    monkeypatch.setenv("MTTKRP_KEY_ORDER", "sideways")     # unknown key-order policy: an error, not a silent default
+    with pytest.raises(P.MttkrpError) as e:
+        P.mttkrp_workspace_bytes([1000, 800, 600], 100_000)
+    assert e.value.status == 1 and "MTTKRP_KEY_ORDER" in str(e.value)
+    for ok in ("revcyclic", "desc", "asc", "cyclic"):
+        monkeypatch.setenv("MTTKRP_KEY_ORDER", ok)
+        assert P.mttkrp_workspace_bytes([1000, 800, 600], 100_000) > 0
+
+
 def test_null_arguments_return_status_not_crash(lib):
     out = ctypes.c_void_p(None)
     dims = (ctypes.c_int64 * 3)(5, 4, 3)
