@@ -318,8 +318,7 @@ __global__ void k_build_records(const int32_t* __restrict__ idx, const float* __
     uint32_t* r = rec + (size_t)k * (N + 1);
     for (int l = 0; l < N; ++l) {
         uint32_t key = (uint32_t)idx[(size_t)order.v[l] * nnz + src];
-        if (l >= 1 && l <= N - 2) key |= ((f >> l) & 1u) << 31;
-        if (l == N - 1) key |= (f & 1u) << 31;
+        if (l <= N - 2) key |= ((f >> l) & 1u) << 31;                  // e_l rides on key word l (common.cuh)
         r[l] = key;
     }
     r[N] = k < nnz ? __float_as_uint(vals[src]) : 0u;
@@ -473,7 +472,7 @@ mttkrp_status_t plan_layouts(int N, const int64_t* dims, int64_t nnz, LayoutPlan
             lp->pk[d].off[l] = (l < N - 1) ? off : 0;
             if (l < N - 1) off += b;
         }
-        if (off > 64 || lp->pk[d].bits[N - 1] + (N - 1) > 32) packed = false;
+        if (off + (N - 1) > 64) packed = false;                       // keys of levels 0..N-2 + N-1 flags in 64 bits
     }
     lp->packed = packed ? 1 : 0;
     lp->rec_words = packed ? 4 : N + 1;

@@ -32,11 +32,12 @@ void set_error(const char* fmt, ...);
     } while (0)
 
 // Run-end flags.  A record of the mode-d layout is N uint32 key words (k_0 = i_d first) + the fp32
-// value.  Indices are < 2^31, so bit 31 of a key word is free; the format builder and the remap pass
+// value.  Indices are < 2^28, so bit 31 of a key word is free; the format builder and the remap pass
 // store there, for the record at position j, e_l = "record j+1 differs from record j in one of the
-// keys k_0..k_l" (the run of equal (k_0..k_l) ends at j):  e_l sits in word l for 1 <= l <= N-2 and
-// e_0 (the output row ends) in word N-1.  Word 0 is never flagged.  Padding records repeat the keys of
-// the last nonzero (no run ends); the very last record of the padded array has every flag set.
+// keys k_0..k_l" (the run of equal (k_0..k_l) ends at j): e_l sits in bit 31 of word l for
+// 0 <= l <= N-2.  The last key word (the row gathered for every nonzero) carries no flag, so the hot
+// loop turns it into an address with one multiply-add.  Padding records repeat the keys of the last
+// nonzero (no run ends); the very last record of the padded array has every flag set.
 constexpr uint32_t kFlag = 0x80000000u;
 constexpr uint32_t kKeyMask = 0x7fffffffu;
 
@@ -45,16 +46,15 @@ constexpr uint32_t kKeyMask = 0x7fffffffu;
 template <int N>
 __device__ __forceinline__ void apply_run_flags(uint32_t* k, uint32_t f) {
 #pragma unroll
-    for (int l = 1; l < N - 1; ++l) k[l] |= ((f >> l) & 1u) << 31;
-    k[N - 1] |= (f & 1u) << 31;
+    for (int l = 0; l < N - 1; ++l) k[l] |= ((f >> l) & 1u) << 31;
 }
 
 // Packed 16-byte records (N >= 4).  When the index widths allow, a record is {w0, w1, w2, val}: the keys of
-// levels 0..N-2 are a bit string in the 64 bits (w1:w0) (level l at bit off[l], bits[l] wide), the last
-// key sits in the low bits of w2 and the N-1 run-end flags in its top bits (e_l at bit 32-(N-1)+l).
-// This is the paper's bit-level size accounting applied to the hot-path record: the
-// remap then moves one 128-bit word per nonzero whatever N is.  Needs bits[N-1] + N-1 <= 32 and
-// sum_{l<N-1} bits[l] <= 64 in every layout; otherwise the handle keeps 4*(N+1)-byte records.
+// levels 0..N-2 are a bit string in the low bits of the 64-bit word (w1:w0) (level l at bit off[l], bits[l]
+// wide), the N-1 run-end flags sit in its top bits (e_l at bit 63-l, i.e. bit 31-l of w1), and w2 is the last
+// key, flag-free.  This is the paper's bit-level size accounting applied to the hot-path
+// record: the remap then moves one 128-bit word per nonzero whatever N is.  Needs
+// sum_{l<N-1} bits[l] + (N-1) <= 64 in every layout; otherwise the handle keeps 4*(N+1)-byte records.
 struct PackDesc {
     int32_t bits[kMaxModes];
     int32_t off[kMaxModes];
@@ -67,8 +67,8 @@ template <int N>
 __device__ __forceinline__ uint4 pk_pack(const uint32_t* k, uint32_t flags, uint32_t val, const PackDesc& d) {
     uint64_t w01 = 0;
 #pragma unroll
-    for (int l = 0; l < N - 1; ++l) w01 |= (uint64_t)k[l] << d.off[l];
-    return make_uint4((uint32_t)w01, (uint32_t)(w01 >> 32), k[N - 1] | (flags << (32 - (N - 1))), val);
+    for (int l = 0; l < N - 1; ++l) w01 |= ((uint64_t)k[l] << d.off[l]) | ((uint64_t)((flags >> l) & 1u) << (63 - l));
+    return make_uint4((uint32_t)w01, (uint32_t)(w01 >> 32), k[N - 1], val);
 }
 
 // Per-mode tables built by mttkrp_create.

@@ -5,10 +5,10 @@
 // Layout: records sorted by the key tuple (k_0 = i_d, k_1, ..., k_{N-1}); record = N uint32 keys in
 // that order + fp32 value, or (N >= 4, PACKED) 16 bytes with the keys bit-packed (common.cuh PackDesc).
 // The record carries the run-end flags that the format builder and the remap pass derived from the
-// sorted order (bit 31 of the key words / top bits of w2, common.cuh), so it is self-contained: the hot
-// loop has no look-ahead compare.
+// sorted order (bit 31 of key words 0..N-2 / top bits of w1, common.cuh), so it is self-contained: the
+// hot loop has no look-ahead compare, and the last key word is flag-free (one multiply-add -> address).
 // A thread block owns one shard = shard_nnz consecutive records (equal-nnz shards).  Inside the
-// block a GROUP of R/V lanes (V = 4 rank columns per lane, one 128-bit LDG per factor row per lane:
+// block a GROUP of R/4 lanes (4 rank columns per lane, one 128-bit LDG per factor row per lane:
 // a warp instruction then covers whole 128-byte lines, one L1 wavefront each) walks a contiguous
 // chunk of the shard one nonzero at a time:
 //   l(r) = val * prod_w A_w[i_w, r]         (Alg. 2 lines 8-13)
@@ -21,8 +21,10 @@
 // records per group, interleaved by group so one LDS.128 serves all groups without bank conflicts).
 // D steps ahead of the arithmetic the group reads its record from the ring and issues the
 // factor-row gathers for that step into rotating registers.  The arithmetic is packed fp32x2 FMA.
-// The kernel is bound by the L1 data pipe (one wavefront per gathered line), so every other use of
-// that pipe is kept minimal: one cp.async and one LDS per record.
+// The kernel is bound by the L1 data pipe (one 128-byte wavefront per clock per SM; every gathered row
+// is one) and, next, by instruction issue, so the loop body is kept to what the data needs
+// (profiles/r2_sass_hot_loop.md): one LDS.128 per record, one multiply-add per row address, sign tests
+// for the flags, and a warp-uniform branch (one vote) around the rare output-row end.
 //
 // Rows that begin and end inside a chunk are stored with plain stores by their only owner
 // (Observation 2: no global atomics).  The first/last partial rows of each chunk
@@ -45,7 +47,7 @@ struct KernelArgs {
     float* out;
     float* carry;            // [2*num_shards][R]
     uint32_t kmask[N];       // packed records (common.cuh PackDesc): mask and bit offset of the key of level l;
-    int32_t koff[N];         // kmask[0] also masks word 0 of unpacked records (all ones)
+    int32_t koff[N];         // unpacked: kmask[l] = kKeyMask
 };
 
 // ---- small PTX helpers ------------------------------------------------------------------------
@@ -63,16 +65,13 @@ __device__ __forceinline__ float2 splat2(float s) {
     return *reinterpret_cast<float2*>(&d);
 }
 
-template <int V>
-struct Vec {                 // V rank columns of one lane, as fp32 pairs
-    float2 p[V / 2];
+struct Vec {                 // 4 rank columns of one lane, as fp32 pairs
+    float2 p[2];
 };
-
-template <int V>
-__device__ __forceinline__ Vec<V> vzero() {
-    Vec<V> r;
-#pragma unroll
-    for (int i = 0; i < V / 2; ++i) r.p[i] = make_float2(0.f, 0.f);
+__device__ __forceinline__ Vec vzero() {
+    Vec r;
+    r.p[0] = make_float2(0.f, 0.f);
+    r.p[1] = make_float2(0.f, 0.f);
     return r;
 }
 
@@ -85,46 +84,42 @@ __device__ __forceinline__ uint64_t l2_policy_evict_first() {
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
     return p;
 }
-// One lane's V columns of a factor row (read-only path; 128-bit or 256-bit load).
-// `base` = factor matrix (uniform), `word` = row index with bit 31 (run-end flag) ignored, `sub` = this
-// lane's slot inside the row.  The element offset (row * R/V + sub) is formed in 32 bits - the shift
-// drops the flag bit - and scaled by one 32x32->64 multiply-add on the uniform base, so a row address
-// costs two instructions and no per-lane pointer registers.  Needs dims[m] < 2^28 (api.cu check_shape).
-template <int V, int R>
-__device__ __forceinline__ Vec<V> ld_row(const float* __restrict__ base, uint32_t word, uint32_t sub) {
-    constexpr int SH = (R / V == 16) ? 4 : (R / V == 8) ? 3 : (R / V == 4) ? 2 : 1;      // log2(lanes per row)
+// One lane's 4 columns of a factor row (read-only path, 128-bit load).  `base` = this lane's slot in row 0 of
+// the factor matrix (float4 units), `key` = row index, LPN = lanes per row: the address is one 32x32->64
+// multiply-add on a per-lane base.  Needs dims[m] < 2^28 (api.cu check_shape).
+template <int LPN>
+__device__ __forceinline__ Vec ld_row(const float4* __restrict__ base, uint32_t key) {
+    const float4 v = __ldg(base + (size_t)key * LPN);
+    Vec r;
+    r.p[0] = make_float2(v.x, v.y);
+    r.p[1] = make_float2(v.z, v.w);
+    return r;
+}
+// Same for a key word that still carries its run-end flag in bit 31 (fiber levels): the element offset
+// (word * LPN + sub) is formed in 32 bits - the shift drops the flag - and scaled by one multiply-add on the
+// uniform base, so no mask and no per-lane pointer registers are needed.
+template <int LPN>
+__device__ __forceinline__ Vec ld_row_flagged(const float* __restrict__ base, uint32_t word, uint32_t sub) {
+    constexpr int SH = LPN == 16 ? 4 : (LPN == 8 ? 3 : (LPN == 4 ? 2 : 1));
     const uint32_t off = (word << SH) + sub;
-    Vec<V> r;
-    if constexpr (V == 8) {
-        const float* p = base + (size_t)off * 8;
-        asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                     : "=f"(r.p[0].x), "=f"(r.p[0].y), "=f"(r.p[1].x), "=f"(r.p[1].y), "=f"(r.p[2].x), "=f"(r.p[2].y),
-                       "=f"(r.p[3].x), "=f"(r.p[3].y)
-                     : "l"(p));
-    } else {
-        const float4 v = __ldg(reinterpret_cast<const float4*>(base) + off);
-        r.p[0] = make_float2(v.x, v.y);
-        r.p[1] = make_float2(v.z, v.w);
-    }
+    const float4 v = __ldg(reinterpret_cast<const float4*>(base) + off);
+    Vec r;
+    r.p[0] = make_float2(v.x, v.y);
+    r.p[1] = make_float2(v.z, v.w);
     return r;
 }
 // acc += a * b (elementwise), acc += s * b
-template <int V>
-__device__ __forceinline__ void vfma(Vec<V>& acc, const Vec<V>& a, const Vec<V>& b) {
-#pragma unroll
-    for (int i = 0; i < V / 2; ++i) acc.p[i] = ffma2(a.p[i], b.p[i], acc.p[i]);
+__device__ __forceinline__ void vfma(Vec& acc, const Vec& a, const Vec& b) {
+    acc.p[0] = ffma2(a.p[0], b.p[0], acc.p[0]);
+    acc.p[1] = ffma2(a.p[1], b.p[1], acc.p[1]);
 }
-template <int V>
-__device__ __forceinline__ void vfmas(Vec<V>& acc, float s, const Vec<V>& b) {
+__device__ __forceinline__ void vfmas(Vec& acc, float s, const Vec& b) {
     const float2 ss = splat2(s);
-#pragma unroll
-    for (int i = 0; i < V / 2; ++i) acc.p[i] = ffma2(ss, b.p[i], acc.p[i]);
+    acc.p[0] = ffma2(ss, b.p[0], acc.p[0]);
+    acc.p[1] = ffma2(ss, b.p[1], acc.p[1]);
 }
-template <int V>
-__device__ __forceinline__ void vstore(float* dst, const Vec<V>& v) {
-#pragma unroll
-    for (int i = 0; i < V / 4; ++i)
-        *reinterpret_cast<float4*>(dst + 4 * i) = make_float4(v.p[2 * i].x, v.p[2 * i].y, v.p[2 * i + 1].x, v.p[2 * i + 1].y);
+__device__ __forceinline__ void vstore(float* dst, const Vec& v) {
+    *reinterpret_cast<float4*>(dst) = make_float4(v.p[0].x, v.p[0].y, v.p[1].x, v.p[1].y);
 }
 
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, uint64_t policy) {
@@ -144,13 +139,26 @@ __device__ __forceinline__ void cp_async4(uint32_t dst, const void* src) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int NPEND>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(NPEND) : "memory"); }
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ uint32_t lds32(uint32_t addr) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
 
 // ---- compile-time geometry ---------------------------------------------------------------------
-#ifndef MK_V8
-#define MK_V8 0          // 1: 8 columns per lane (256-bit gathers); measured 1.4 L1 wavefronts per 128-byte line
-#endif                   //    against 1.0 for 128-bit gathers
-#ifndef MK_D
+#ifndef MK_D             // gather look-ahead of the default variant, in steps
 #define MK_D 2
+#endif
+#ifndef MK_D_DEEP        // ... of the DEEP variant
+#define MK_D_DEEP 4
+#endif
+#ifndef MK_OPAQUE
+#define MK_OPAQUE 1
 #endif
 #ifndef MK_STAGES
 #define MK_STAGES 3
@@ -158,9 +166,12 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 #ifndef MK_MINB          // resident blocks per SM the register allocation must allow; 0 = per-N default below.
 #define MK_MINB 0        // Measured on B200 (configs[1], configs[2]): occupancy beats deeper look-ahead.
 #endif
+#ifndef MK_MINB_DEEP
+#define MK_MINB_DEEP 0
+#endif
 template <int N, int R, bool DEEP, bool PACKED>
 struct Geo {
-    static constexpr int V = (MK_V8 && R >= 16) ? 8 : 4; // rank columns per lane
+    static constexpr int V = 4;                          // rank columns per lane
     static constexpr int LPN = R / V;                    // lanes per nonzero (group size)
     static constexpr int NPW = 32 / LPN;                 // groups per warp
     static constexpr int WARPS = kBlockThreads / 32;
@@ -169,15 +180,16 @@ struct Geo {
     static constexpr int SLOTW = (RECW + 3) / 4 * 4;     // ring slot words (16-byte multiple)
     static constexpr int K = (NPW * SLOTW <= 32) ? 8 : 4;  // records per group per ring stage
     static constexpr int STAGES = MK_STAGES;             // round r computing, r+1 landed, the rest in flight
-    // gather look-ahead, in steps (K % D == 0).  DEEP: twice the look-ahead at one block per SM less, for
+    // gather look-ahead, in steps (K % D == 0).  DEEP: twice the look-ahead at fewer blocks per SM, for
     // factor matrices that do not fit L2 (every gather that misses is a random HBM access).
-    static constexpr int D0 = (DEEP && N <= 3) ? 2 * MK_D : MK_D;
+    static constexpr int D0 = (DEEP && N <= 3) ? MK_D_DEEP : MK_D;
     static constexpr int D = (D0 < K) ? D0 : K / 2;
     static constexpr int RING_WORDS = STAGES * K * NPW * SLOTW;        // per warp
     static constexpr int ENT_WORDS = 2 * NPW * R;                       // per warp: first/last partial rows
     static constexpr int WARP_WORDS = RING_WORDS > ENT_WORDS ? RING_WORDS : ENT_WORDS;
     static constexpr int NL = N - 1;                     // accumulator levels t[0..NL-1]
-    static constexpr int MINB = MK_MINB ? MK_MINB : (N <= 3 ? (DEEP ? 4 : 5) : (N == 4 ? 4 : 3));
+    static constexpr int MINB_DEF = N <= 3 ? (DEEP ? 3 : 5) : (N == 4 ? 4 : (N <= 6 ? 3 : 2));
+    static constexpr int MINB = DEEP ? (MK_MINB_DEEP ? MK_MINB_DEEP : MINB_DEF) : (MK_MINB ? MK_MINB : MINB_DEF);
     static constexpr int SMEM_BYTES = 4 * (WARPS * WARP_WORDS + WARPS * NPW * R + 2 * WARPS * R + WARPS * 2 * NPW + 2 * WARPS);
 };
 
@@ -245,134 +257,290 @@ __global__ void __launch_bounds__(kBlockThreads, Geo<N, R, DEEP, PACKED>::MINB) 
 
     uint32_t* const ring = &s_warp[warp][0];
     const uint32_t* const ring_g = ring + g * SLOTW;      // this group's column of the ring
-    const uint32_t ring_gs = (uint32_t)__cvta_generic_to_shared(ring_g);
+    uint32_t ring_gs = (uint32_t)__cvta_generic_to_shared(ring_g);
+#if MK_OPAQUE
+    asm volatile("mov.u32 %0, %0;" : "+r"(ring_gs));     // opaque: kept in a register instead of being re-derived from %tid every round
+#endif
 
-    const uint64_t rec_policy = l2_policy_evict_first();
-    auto issue_round = [&](int r) {
-        if (r < nrounds) {
-            const uint32_t* src = grec + (size_t)r * (K * RECW);
-            const uint32_t dst = ring_gs + 4u * (uint32_t)((r % STAGES) * STAGEW);
+    // per-lane bases of the factor rows: row r of level l = fb[l] + r * LPN (float4 units)
+    const float4* fb[N];
 #pragma unroll
-            for (int i = 0; i < NPIECE; ++i) {
-                const int p = sub + i * LPN;
-                if (p < K * PPR) {
-                    const int jj = p / PPR, q = p % PPR;
-                    const uint32_t d2 = dst + 4u * (uint32_t)(jj * ROWW + q * PW);
-                    if constexpr (PW == 4) cp_async16(d2, src + jj * RECW + q * PW, rec_policy);
-                    else if constexpr (PW == 2) cp_async8(d2, src + jj * RECW + q * PW);
-                    else cp_async4(d2, src + jj * RECW + q * PW);
+    for (int l = 1; l < N; ++l) fb[l] = reinterpret_cast<const float4*>(a.fac[l]) + sub;
+#if MK_OPAQUE >= 2
+    // Register-resident base of the deepest fiber level: without it every fiber-row gather reloads the pointer
+    // from the constant bank (LDC), which costs an issue slot and, worse, one of the six scoreboards.
+    const float* fiber_base = NL >= 2 ? a.fac[NL >= 2 ? NL - 1 : 1] : nullptr;
+    if constexpr (NL >= 2) asm volatile("mov.u64 %0, %0;" : "+l"(fiber_base));
+#else
+    const float* fiber_base = NL >= 2 ? a.fac[NL >= 2 ? NL - 1 : 1] : nullptr;
+#endif
+
+    // ---- record ring fill ---------------------------------------------------------------------------------
+    const uint64_t rec_policy = l2_policy_evict_first();
+    // 16-byte records: piece p of the round = record p of the group, copied by lane p % LPN; the source
+    // pointer just advances by one round per call.
+    const uint32_t* fill_src = grec + (size_t)sub * RECW;
+    uint32_t fill_dst = ring_gs + 4u * (uint32_t)(sub * ROWW);           // ring slot of record `sub` in stage 0
+#if MK_OPAQUE
+    asm volatile("mov.u32 %0, %0;" : "+r"(fill_dst));
+#endif
+    int fill_round = 0, fill_stage = 0;
+    auto issue_round = [&]() {
+        if (fill_round < nrounds) {
+            const uint32_t dst = ring_gs + 4u * (uint32_t)(fill_stage * STAGEW);
+            if constexpr (PPR == 1) {
+                const uint32_t dl = fill_dst + 4u * (uint32_t)(fill_stage * STAGEW);
+#pragma unroll
+                for (int i = 0; i < NPIECE; ++i) {
+                    const int p = sub + i * LPN;
+                    if (NPIECE * LPN == K || p < K) cp_async16(dl + 4u * (uint32_t)(i * LPN * ROWW), fill_src + (size_t)i * LPN * RECW, rec_policy);
+                }
+                fill_src += K * RECW;
+            } else {
+                const uint32_t* src = grec + (size_t)fill_round * (K * RECW);
+#pragma unroll
+                for (int i = 0; i < NPIECE; ++i) {
+                    const int p = sub + i * LPN;
+                    if (p < K * PPR) {
+                        const int jj = p / PPR, q = p % PPR;
+                        const uint32_t d2 = dst + 4u * (uint32_t)(jj * ROWW + q * PW);
+                        if constexpr (PW == 2) cp_async8(d2, src + jj * RECW + q * PW);
+                        else cp_async4(d2, src + jj * RECW + q * PW);
+                    }
                 }
             }
         }
+        ++fill_round;
+        fill_stage = (fill_stage + 1 == STAGES) ? 0 : fill_stage + 1;
         cp_async_commit();
     };
-    auto read_slot = [&](const uint32_t* slot, uint32_t* w) {
-        const uint4* p = reinterpret_cast<const uint4*>(slot);
-#pragma unroll
-        for (int i = 0; i < SLOTW / 4; ++i) {
-            const uint4 v = p[i];
-            w[4 * i] = v.x; w[4 * i + 1] = v.y; w[4 * i + 2] = v.z; w[4 * i + 3] = v.w;
-        }
-    };
 
-    Vec<V> t[NL];                                         // t[0] = output row accumulator
+    Vec t[NL];                                            // t[0] = output row accumulator
 #pragma unroll
-    for (int l = 0; l < NL; ++l) t[l] = vzero<V>();
-    Vec<V> al[D];                                         // last-level rows for the D steps in flight
-    Vec<V> rb[NL][D];                                     // rb[l][slot]: row of level l, gathered at the end of its run
-    float val[D];
-    uint32_t fl[D];                                       // bit l: the run of level l ends at this step
-    int seg = 0;                                          // output-row segments finished in this chunk
-
-    // Issue the gathers of one step whose record sits at `slot`.  The record carries its run-end
-    // flags (common.cuh).  The chunk's last record closes every inner run and leaves the output row
-    // open: it is finished by the epilogue, which knows whether the row continues in the next chunk.
-    auto prefetch = [&](const uint32_t* slot, int s, bool chunk_last) {
-        uint32_t w[SLOTW];
-        read_slot(slot, w);
-        if constexpr (PACKED) {                           // {w0, w1, w2 = flags | last key, val}
-            uint32_t f = w[2] >> (32 - (N - 1));
-            if (chunk_last) f = (f | ((1u << NL) - 2u)) & ~1u;
-            al[s] = ld_row<V, R>(a.fac[N - 1], w[2] & a.kmask[N - 1], sub);
-#pragma unroll
-            for (int l = 1; l < NL; ++l)
-                if (f & (1u << l)) rb[l][s] = ld_row<V, R>(a.fac[l], pk_get(w[0], w[1], a.koff[l], a.kmask[l]), sub);
-            val[s] = __uint_as_float(w[3]);
-            fl[s] = f;
+    for (int l = 0; l < NL; ++l) t[l] = vzero();
+    bool first_done = false;                              // the chunk's first output-row segment has been emitted
+    // Emits the output row that ends at the record whose word 0 is `w0` (run-end flag masked off by the caller's test).
+    auto emit_row = [&](uint32_t row) {
+        if (!first_done) {
+            vstore(&s_first[warp][g][sub * V], t[0]);
+            if (sub == 0) s_erow[warp][2 * g] = (int)row;
         } else {
-            if (chunk_last) {
-#pragma unroll
-                for (int l = 1; l < NL; ++l) w[l] |= kFlag;
-                w[N - 1] &= kKeyMask;
-            }
-            al[s] = ld_row<V, R>(a.fac[N - 1], w[N - 1], sub);
-            uint32_t f = w[N - 1] >> 31;
-#pragma unroll
-            for (int l = 1; l < NL; ++l) {
-                if (w[l] & kFlag) rb[l][s] = ld_row<V, R>(a.fac[l], w[l], sub);
-                f |= (w[l] >> 31) << l;
-            }
-            val[s] = __uint_as_float(w[N]);
-            fl[s] = f;
+            vstore(a.out + (size_t)row * R + sub * V, t[0]);
         }
+        first_done = true;
+        t[0] = vzero();
     };
-    // Arithmetic of one step (its record sits at `slot`).
-    auto compute = [&](const uint32_t* slot, int s) {
-        const uint32_t e = fl[s];
-        vfmas<V>(t[NL - 1], val[s], al[s]);
+    constexpr bool BATCH = DEEP && N <= 3 && K == 8 && !PACKED;
+    if constexpr (BATCH) {
+        // ---- batch variant (N <= 3) -------------------------------------------------------------------------
+        // ptxas tracks every factor-row LDG of this loop on ONE scoreboard, so any wait drains all gathers in
+        // flight: a software pipeline degenerates into "issue, wait for everything, compute"
+        // (profiles/r2_scoreboards.md).  This variant makes that structure explicit and deep: the records of B = 4
+        // steps are read with back-to-back LDS.128, their B last-level rows and up to B fiber rows are requested
+        // together (up to 8 independent 128-bit gathers per lane in flight), then the B steps are computed.  Costs
+        // 64 registers (4 blocks per SM); one vote per batch replaces the per-step output-row-end test.
+        constexpr int B = 4;
+        Vec al[B], rb[B];
+        float val[B];
+        bool e1[B];
+        uint32_t anyend = 0;                              // OR of the batch's word 0: sign set = some output row ends in it
+        auto P = [&](uint32_t base) {                     // `base` = ring byte address of the batch's first record
+            uint4 q[B];
 #pragma unroll
-        for (int l = NL - 1; l >= 1; --l) {
-            if (e & (1u << l)) {
-                vfma<V>(t[l - 1], rb[l][s], t[l]);
-                t[l] = vzero<V>();
+            for (int s = 0; s < B; ++s) q[s] = lds128(base + 4u * (uint32_t)(s * ROWW));
+            anyend = 0;
+#pragma unroll
+            for (int s = 0; s < B; ++s) {
+                if constexpr (N == 3) {
+                    al[s] = ld_row<LPN>(fb[2], q[s].z);
+                    e1[s] = (int32_t)q[s].y < 0;
+                    if (e1[s]) rb[s] = ld_row_flagged<LPN>(fiber_base, q[s].y, sub);
+                    val[s] = __uint_as_float(q[s].w);
+                } else {
+                    al[s] = ld_row<LPN>(fb[1], q[s].y);
+                    e1[s] = false;
+                    val[s] = __uint_as_float(q[s].z);
+                }
+                anyend |= q[s].x;
             }
-        }
-        if (e & 1u) {                                     // an output row ends inside the chunk
-            const uint32_t row = slot[0] & a.kmask[0];
-            if (seg == 0) {
-                vstore<V>(&s_first[warp][g][sub * V], t[0]);
-                if (sub == 0) s_erow[warp][2 * g] = (int)row;
+        };
+        auto C = [&](uint32_t base) {
+            if (!__any_sync(0xffffffffu, (int32_t)anyend < 0)) {      // common: no output row ends in this batch
+#pragma unroll
+                for (int s = 0; s < B; ++s) {
+                    vfmas(t[NL - 1], val[s], al[s]);
+                    if constexpr (N == 3) {
+                        if (e1[s]) { vfma(t[0], rb[s], t[1]); t[1] = vzero(); }
+                    }
+                }
             } else {
-                vstore<V>(a.out + (size_t)row * R + sub * V, t[0]);
+#pragma unroll
+                for (int s = 0; s < B; ++s) {
+                    vfmas(t[NL - 1], val[s], al[s]);
+                    if constexpr (N == 3) {
+                        if (e1[s]) { vfma(t[0], rb[s], t[1]); t[1] = vzero(); }
+                    }
+                    const uint32_t w0 = lds32(base + 4u * (uint32_t)(s * ROWW));
+                    if ((int32_t)w0 < 0) emit_row(w0 & kKeyMask);
+                }
             }
-            ++seg;
-            t[0] = vzero<V>();
-        }
-    };
-
-    // ---- prologue: rounds 0..AHEAD-1 in flight, round 0 landed ----------------------------------------
+        };
 #pragma unroll
-    for (int r = 0; r < AHEAD; ++r) issue_round(r);
-    cp_async_wait<AHEAD - 1>();                           // round 0 has landed
-    __syncwarp();
-#pragma unroll
-    for (int i = 0; i < D; ++i) prefetch(ring_g + i * ROWW, i, false);
-    for (int r = 0; r < nrounds; ++r) {
-        issue_round(r + AHEAD);                           // reuses the stage of round r-1
-        cp_async_wait<AHEAD - 1>();                       // rounds <= r+1 have landed
+        for (int r = 0; r < AHEAD; ++r) issue_round();
+        cp_async_wait<AHEAD - 1>();                       // round 0 has landed
         __syncwarp();
-        const uint32_t* cs = ring_g + (r % STAGES) * STAGEW;            // this round's stage
-        const uint32_t* ns = ring_g + ((r + 1) % STAGES) * STAGEW;      // next round's stage
-        const bool more = r + 1 < nrounds;
-#pragma unroll
-        for (int i = 0; i < K; ++i) {
-            compute(cs + i * ROWW, i % D);
-            if (i + D < K) prefetch(cs + (i + D) * ROWW, i % D, (i + D == K - 1) && !more);
-            else if (more) prefetch(ns + (i + D - K) * ROWW, i % D, false);
+        P(ring_gs);
+        int stage = 0;
+        for (int r = 0; r < nrounds; ++r) {
+            issue_round();                                // round r+AHEAD, reuses the stage of round r-1
+            cp_async_wait<AHEAD - 1>();                   // rounds <= r+1 have landed
+            __syncwarp();
+            const int nstage = (stage + 1 == STAGES) ? 0 : stage + 1;
+            const uint32_t cs = ring_gs + 4u * (uint32_t)(stage * STAGEW);
+            const uint32_t ns = ring_gs + 4u * (uint32_t)(nstage * STAGEW);
+            C(cs);
+            P(cs + 4u * (uint32_t)(B * ROWW));
+            C(cs + 4u * (uint32_t)(B * ROWW));
+            if (r + 1 < nrounds) P(ns);
+            stage = nstage;
+            __syncwarp();                                 // everyone is done with round r's stage
         }
-        __syncwarp();                                     // everyone is done with round r's stage
+    } else {
+        Vec al[D];                                            // last-level rows for the D steps in flight
+        Vec rb[NL][D];                                        // rb[l][slot]: row of level l, gathered at the end of its run
+        float val[D];
+        bool e[NL][D];                                        // e[l][slot]: the run of level l ends at that step
+
+        // Issue the gathers of one step whose record sits at ring byte address `slot`.
+        auto prefetch = [&](uint32_t slot, int s) {
+            uint32_t w[SLOTW];
+#pragma unroll
+            for (int i = 0; i < SLOTW / 4; ++i) {
+                const uint4 v = lds128(slot + 16u * i);
+                w[4 * i] = v.x; w[4 * i + 1] = v.y; w[4 * i + 2] = v.z; w[4 * i + 3] = v.w;
+            }
+            if constexpr (PACKED) {                           // {w0, w1 = flags | keys, w2 = last key, val}
+                al[s] = ld_row<LPN>(fb[N - 1], w[2]);
+#pragma unroll
+                for (int l = 0; l < NL; ++l) e[l][s] = (w[1] & (0x80000000u >> l)) != 0;
+                if (__any_sync(0xffffffffu, e[NL - 1][s])) {
+#pragma unroll
+                    for (int l = 1; l < NL; ++l)
+                        if (e[l][s]) rb[l][s] = ld_row<LPN>(fb[l], pk_get(w[0], w[1], a.koff[l], a.kmask[l]));
+                }
+                val[s] = __uint_as_float(w[3]);
+            } else {
+                al[s] = ld_row<LPN>(fb[N - 1], w[N - 1]);
+#pragma unroll
+                for (int l = 0; l < NL; ++l) e[l][s] = (int32_t)w[l] < 0;
+                if constexpr (NL >= 2) {
+                    if (e[NL - 1][s]) rb[NL - 1][s] = ld_row_flagged<LPN>(fiber_base, w[NL - 1], sub);
+                }
+                if constexpr (NL >= 3) {                      // e_l implies e_{l+1}: one vote guards all upper levels
+                    if (__any_sync(0xffffffffu, e[NL - 2][s])) {
+#pragma unroll
+                        for (int l = 1; l < NL - 1; ++l)
+                            if (e[l][s]) rb[l][s] = ld_row_flagged<LPN>(a.fac[l], w[l], sub);
+                    }
+                }
+                val[s] = __uint_as_float(w[N]);
+            }
+        };
+        // Arithmetic of one step (its record sits at `slot`).
+        auto compute = [&](uint32_t slot, int s) {
+            vfmas(t[NL - 1], val[s], al[s]);
+            if constexpr (NL >= 2) {
+                if (e[NL - 1][s]) {
+                    vfma(t[NL - 2], rb[NL - 1][s], t[NL - 1]);
+                    t[NL - 1] = vzero();
+                }
+            }
+            if constexpr (NL >= 3) {
+                if (__any_sync(0xffffffffu, e[NL - 2][s])) {
+#pragma unroll
+                    for (int l = NL - 2; l >= 1; --l) {
+                        if (e[l][s]) {
+                            vfma(t[l - 1], rb[l][s], t[l]);
+                            t[l] = vzero();
+                        }
+                    }
+                }
+            }
+            if (__any_sync(0xffffffffu, e[0][s])) {           // rare: an output row ends inside the chunk
+                // Every lane reads its group's row id first (a volatile load): the branch above then depends on the
+                // vote alone and stays warp-uniform; only the stores below are per lane.
+                uint32_t row;
+                if constexpr (PACKED) row = pk_get(lds32(slot), lds32(slot + 4), a.koff[0], a.kmask[0]);
+                else row = lds32(slot) & kKeyMask;
+                if (e[0][s]) emit_row(row);
+            }
+        };
+
+        // ---- prologue: rounds 0..AHEAD-1 in flight, round 0 landed ----------------------------------------
+#pragma unroll
+        for (int r = 0; r < AHEAD; ++r) issue_round();
+        cp_async_wait<AHEAD - 1>();                           // round 0 has landed
+        __syncwarp();
+#pragma unroll
+        for (int i = 0; i < D; ++i) prefetch(ring_gs + 4u * (uint32_t)(i * ROWW), i);
+        int stage = 0;                                        // r % STAGES
+        for (int r = 0; r < nrounds; ++r) {
+            issue_round();                                    // round r+AHEAD, reuses the stage of round r-1
+            cp_async_wait<AHEAD - 1>();                       // rounds <= r+1 have landed
+            __syncwarp();
+            const int nstage = (stage + 1 == STAGES) ? 0 : stage + 1;
+            const uint32_t cs = ring_gs + 4u * (uint32_t)(stage * STAGEW);            // this round's stage
+            const uint32_t ns = ring_gs + 4u * (uint32_t)(nstage * STAGEW);           // next round's stage
+            const bool more = r + 1 < nrounds;
+#pragma unroll
+            for (int i = 0; i < K; ++i) {
+                compute(cs + 4u * (uint32_t)(i * ROWW), i % D);
+                if (i + D < K) prefetch(cs + 4u * (uint32_t)((i + D) * ROWW), i % D);
+                else if (more) prefetch(ns + 4u * (uint32_t)((i + D - K) * ROWW), i % D);
+            }
+            stage = nstage;
+            __syncwarp();                                     // everyone is done with round r's stage
+        }
     }
     cp_async_wait<0>();
-    const uint32_t last_row = ring_g[((nrounds - 1) % STAGES) * STAGEW + (K - 1) * ROWW] & a.kmask[0];
     __syncwarp();
-    // chunk epilogue: the still-open row goes to the first (seg == 0) or last partial-row entry
+    // ---- chunk epilogue -----------------------------------------------------------------------------------
+    // The chunk's last record leaves its inner runs open unless they end there: fold them now (the level's
+    // row is the last record's key), so that t[0] holds everything the chunk contributes to its last row.
+    const uint32_t* const last_rec = ring_g + ((nrounds - 1) % STAGES) * STAGEW + (K - 1) * ROWW;
+    uint32_t lw[SLOTW];
+#pragma unroll
+    for (int i = 0; i < SLOTW; ++i) lw[i] = last_rec[i];
+#pragma unroll
+    for (int l = NL - 1; l >= 1; --l) {
+        bool ended;
+        uint32_t key;
+        if constexpr (PACKED) { ended = (lw[1] & (0x80000000u >> l)) != 0; key = pk_get(lw[0], lw[1], a.koff[l], a.kmask[l]); }
+        else { ended = (int32_t)lw[l] < 0; key = lw[l] & kKeyMask; }
+        if (!ended) {
+            const Vec row = ld_row<LPN>(fb[l], key);
+            vfma(t[l - 1], row, t[l]);
+            t[l] = vzero();
+        }
+    }
+    bool last_open;                                       // the chunk's last output row continues past the chunk
+    uint32_t last_row;
+    if constexpr (PACKED) { last_open = (lw[1] & 0x80000000u) == 0; last_row = pk_get(lw[0], lw[1], a.koff[0], a.kmask[0]); }
+    else { last_open = (int32_t)lw[0] >= 0; last_row = lw[0] & kKeyMask; }
+    __syncwarp();
+    // The still-open row goes to the first (nothing emitted yet) or last partial-row entry; a row that ended
+    // exactly at the chunk's last record was already emitted by the loop.
     float* const s_last = reinterpret_cast<float*>(ring);               // [NPW][R], aliases the ring
-    {
-        float* dst = (seg == 0) ? &s_first[warp][g][sub * V] : s_last + g * R + sub * V;
-        vstore<V>(dst, t[0]);
-        if (sub == 0) {
-            s_erow[warp][2 * g + (seg == 0 ? 0 : 1)] = (int)last_row;
-            if (seg == 0) s_erow[warp][2 * g + 1] = -1;
+    if (last_open) {
+        float* dst = !first_done ? &s_first[warp][g][sub * V] : s_last + g * R + sub * V;
+        vstore(dst, t[0]);
+    }
+    if (sub == 0) {
+        if (last_open) {
+            s_erow[warp][2 * g + (first_done ? 1 : 0)] = (int)last_row;
+            if (!first_done) s_erow[warp][2 * g + 1] = -1;
+        } else {
+            s_erow[warp][2 * g + 1] = -1;                 // first_done here: entry 0 was written by the loop
         }
     }
     if (lane == 0) { s_wrow[2 * warp] = -1; s_wrow[2 * warp + 1] = -1; }
@@ -398,8 +566,8 @@ __global__ void __launch_bounds__(kBlockThreads, Geo<N, R, DEEP, PACKED>::MINB) 
             }
             ++run;
         };
-        for (int e = 0; e < 2 * NPW; ++e) {
-            const int r = s_erow[warp][e];
+        for (int ee = 0; ee < 2 * NPW; ++ee) {
+            const int r = s_erow[warp][ee];
             if (r < 0) continue;
             if (r != cur_row) {
                 if (cur_row >= 0) emit(cur_row, false);
@@ -407,7 +575,7 @@ __global__ void __launch_bounds__(kBlockThreads, Geo<N, R, DEEP, PACKED>::MINB) 
 #pragma unroll
                 for (int q = 0; q < CPL; ++q) acc[q] = 0.f;
             }
-            const float* v = (e & 1) ? s_last + (e >> 1) * R : firsts + (e >> 1) * R;
+            const float* v = (ee & 1) ? s_last + (ee >> 1) * R : firsts + (ee >> 1) * R;
 #pragma unroll
             for (int q = 0; q < CPL; ++q) {
                 const int col = lane + 32 * q;
@@ -420,7 +588,11 @@ __global__ void __launch_bounds__(kBlockThreads, Geo<N, R, DEEP, PACKED>::MINB) 
 
     // level 2: merge the warps' partial rows; rows shared with a neighbouring shard go to the carry buffer
     if (warp == 0) {
-        auto key0_at = [&](int64_t pos) { return __ldg(a.rec + (size_t)pos * RECW) & a.kmask[0]; };   // k_0 sits in word 0
+        auto key0_at = [&](int64_t pos) {
+            const uint32_t* p = a.rec + (size_t)pos * RECW;
+            if constexpr (PACKED) return pk_get(__ldg(p), __ldg(p + 1), a.koff[0], a.kmask[0]);
+            else return __ldg(p) & kKeyMask;                            // k_0 sits in word 0
+        };
         const uint32_t first_row = key0_at(s_begin);
         const uint32_t end_row = key0_at(s_end - 1);
         const bool head_shared = s_begin > 0 && key0_at(s_begin - 1) == first_row;
@@ -497,11 +669,11 @@ static mttkrp_status_t launch_nr(mttkrp_handle_s* h, int d, const float* const* 
         a.out = out;
         a.carry = h->carry;
         // Factor matrices that overflow L2 (126 MB) turn gather misses into random HBM reads: use the
-        // variant with the deeper look-ahead (measured on configs[2]: 2.96 vs 3.19 ms per mode).
+        // variant with the deeper look-ahead.  MTTKRP_FORCE_DEEP (read at create) pins the choice for tests.
         int64_t fac_bytes = 0;
         for (int l = 1; l < N; ++l) fac_bytes += h->dims[mm.order[l]] * (int64_t)R * 4;
         const bool deep = N <= 3 && (h->force_deep >= 0 ? h->force_deep == 1 : fac_bytes > (96ll << 20));
-        for (int l = 0; l < N; ++l) { a.kmask[l] = 0xffffffffu; a.koff[l] = 0; }
+        for (int l = 0; l < N; ++l) { a.kmask[l] = kKeyMask; a.koff[l] = 0; }
         if (h->packed)
             for (int l = 0; l < N; ++l) { a.kmask[l] = pk_mask(mm.pk.bits[l]); a.koff[l] = mm.pk.off[l]; }
         auto launch = [&](auto deep_tag, auto packed_tag) -> mttkrp_status_t {
@@ -510,6 +682,9 @@ static mttkrp_status_t launch_nr(mttkrp_handle_s* h, int d, const float* const* 
             constexpr int smem = Geo<N, R, DEEP, PACKED>::SMEM_BYTES;
             if constexpr (smem > 48 * 1024)               // per device, so not cached in a static
                 MK_CUDA(cudaFuncSetAttribute(k_mttkrp<N, R, DEEP, PACKED>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+#ifdef MK_CARVEOUT                                          // experiment: shared-memory carveout in percent of the maximum
+            MK_CUDA(cudaFuncSetAttribute(k_mttkrp<N, R, DEEP, PACKED>, cudaFuncAttributePreferredSharedMemoryCarveout, MK_CARVEOUT));
+#endif
             TimedLaunch tl(h->timing, kClsMttkrp, st);
             k_mttkrp<N, R, DEEP, PACKED><<<(unsigned)h->num_shards, kBlockThreads, smem, st>>>(a);
             return MTTKRP_OK;
@@ -533,10 +708,12 @@ static mttkrp_status_t launch_nr(mttkrp_handle_s* h, int d, const float* const* 
 template <int N>
 static mttkrp_status_t launch_n(mttkrp_handle_s* h, int d, const float* const* factors, int R, float* out, cudaStream_t st) {
     switch (R) {
+#ifndef MK_FAST_BUILD
         case 8: return launch_nr<N, 8>(h, d, factors, out, st);
         case 16: return launch_nr<N, 16>(h, d, factors, out, st);
-        case 32: return launch_nr<N, 32>(h, d, factors, out, st);
         case 64: return launch_nr<N, 64>(h, d, factors, out, st);
+#endif
+        case 32: return launch_nr<N, 32>(h, d, factors, out, st);
     }
     set_error("unsupported rank %d (8, 16, 32, 64)", R);
     return MTTKRP_EUNSUPPORTED;
@@ -545,13 +722,15 @@ static mttkrp_status_t launch_n(mttkrp_handle_s* h, int d, const float* const* f
 // The resident copy must already be in layout d (api.cu runs the remap passes first).
 mttkrp_status_t launch_mttkrp(mttkrp_handle_s* h, int d, const float* const* factors, int R, float* out, cudaStream_t st) {
     switch (h->N) {
+#ifndef MK_FAST_BUILD                                    // -DMK_FAST_BUILD: N = 3, R = 32 only (SASS inspection)
         case 2: return launch_n<2>(h, d, factors, R, out, st);
-        case 3: return launch_n<3>(h, d, factors, R, out, st);
         case 4: return launch_n<4>(h, d, factors, R, out, st);
         case 5: return launch_n<5>(h, d, factors, R, out, st);
         case 6: return launch_n<6>(h, d, factors, R, out, st);
         case 7: return launch_n<7>(h, d, factors, R, out, st);
         case 8: return launch_n<8>(h, d, factors, R, out, st);
+#endif
+        case 3: return launch_n<3>(h, d, factors, R, out, st);
     }
     set_error("unsupported nmodes %d", h->N);
     return MTTKRP_EUNSUPPORTED;

@@ -98,7 +98,7 @@ __global__ void __launch_bounds__(256) k_remap(const uint32_t* __restrict__ in, 
 // composes, per destination level, where its key sits in the SOURCE record (RemapPk), so the kernel unpacks
 // straight into destination order and repacks with the destination layout's offsets and flags.
 struct RemapPk {
-    int32_t soff[kMaxModes];      // bit offset of the source field in (w1:w0), or -1: it is the low field of w2
+    int32_t soff[kMaxModes];      // bit offset of the source field in (w1:w0), or -1: it is w2 (the last key)
     uint32_t smask[kMaxModes];
 };
 
