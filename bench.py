@@ -354,6 +354,48 @@ def extra_rows(P, W, args, dev, peak, skip_config):
     return rows
 
 
+def alternative_paths(P, W, spec, R, dev, steps):
+    """The two SURVEY.md Sec. 8(f) variants that are kept behind switches because they measured slower, timed on the
+    same workload so that the result is reproducible from the committed code:
+      fused  - MTTKRP_FUSE=1: Alg. 3 executed inside the MTTKRP kernel (the paper's design, Alg. 4 lines 15-19);
+      alg1   - MTTKRP_SHARD_POLICY=alg1: the paper's partitioner, whole rows dealt to kappa = #SM partitions, one thread
+               block per partition, no carry / fix-up."""
+    import torch
+    out = {}
+    os.environ["MTTKRP_FUSE"] = "1"
+    try:
+        case = Case(P, W, spec, R, dev, max_rank=0)
+        if case.info["fused_remap"]:
+            for _ in range(3):
+                case.sweep()
+            ms, _, _ = case.timed_sweeps(steps)
+            k_ms, _, _, brk = case.kernel_classes(steps)
+            out["fused"] = {"ms_per_sweep": ms / steps, "kernel_ms_per_sweep": brk["mttkrp_ms_per_sweep"],
+                            "separate_pass_ms_per_sweep": brk["remap_ms_per_sweep"],
+                            "note": "MTTKRP kernels that also scatter the records into the next layout (Alg. 3 inside Alg. 4)"}
+        case.close()
+    finally:
+        del os.environ["MTTKRP_FUSE"]
+    kappa = torch.cuda.get_device_properties(dev).multi_processor_count
+    os.environ["MTTKRP_SHARD_POLICY"] = "alg1"
+    os.environ["MTTKRP_KAPPA"] = str(kappa)
+    try:
+        case = Case(P, W, spec, R, dev, max_rank=0)
+        case.sweep()
+        ms, _, _ = case.timed_sweeps(1)
+        _, _, _, brk = case.kernel_classes(1)
+        mean = case.nnz / kappa
+        out["alg1"] = {"kappa": kappa, "ms_per_sweep": ms, "mttkrp_ms_per_sweep": brk["mttkrp_ms_per_sweep"],
+                       "remap_ms_per_sweep": brk["remap_ms_per_sweep"], "create_s": case.create_s,
+                       "max_partition_over_mean": [round(x / mean, 2) for x in case.info["max_partition_nnz"]],
+                       "note": "whole rows, longest-first, one thread block per partition (PAPER.md:163-181); one timed sweep"}
+        case.close()
+    finally:
+        del os.environ["MTTKRP_SHARD_POLICY"]
+        del os.environ["MTTKRP_KAPPA"]
+    return out
+
+
 def run_ours(args):
     import torch
     import workloads as W
@@ -452,6 +494,10 @@ def run_ours(args):
     extra = None
     if rank == 0 and world == 1 and not args.no_extra and not args.nnz:
         extra = extra_rows(P, W, args, dev, peak, args.config)
+        alt = alternative_paths(P, W, spec, R, dev, max(5, min(args.steps, 10)))
+        breakdown["fused_ms_per_sweep"] = alt.get("fused", {}).get("ms_per_sweep")
+        breakdown["fused"] = alt.get("fused")
+        breakdown["alg1_policy"] = alt.get("alg1")
 
     cpu_baseline = None
     if want_cpu:

@@ -31,7 +31,9 @@
  *   - Process environment variables read by mttkrp_workspace_bytes / mttkrp_create (test and experiment knobs;
  *     unset = the library decides): MTTKRP_KEY_ORDER = revcyclic|desc|asc|cyclic (anything else: EINVAL),
  *     MTTKRP_PACK = 0|1, MTTKRP_REMAP_BLOCKED = 0|1, MTTKRP_REMAP_BLOCK_LOG2 (clamped to [10,26]),
- *     MTTKRP_FORCE_DEEP = 0|1 (kernel variant).  They must not change between the size query and create.
+ *     MTTKRP_FORCE_DEEP = 0|1 (kernel variant), MTTKRP_FUSE = 0|1 (remap inside the MTTKRP kernel), MTTKRP_SHARD_POLICY = equal|alg1 and MTTKRP_KAPPA (number of
+ *     partitions of the paper's Alg. 1 policy, default one per SM).  They must not change between the size query
+ *     and create.
  */
 #ifndef MTTKRP_B200_H
 #define MTTKRP_B200_H
@@ -80,6 +82,14 @@ typedef struct {
                                             (L2-resident gather window), 0: in destination order */
     double remap_avg_run[MTTKRP_MAX_MODES];
                                          /* average length of the ascending destination runs of that walk */
+    int32_t shard_policy;                /* 0: equal-nnz shards, rows may span blocks (default); 1: the paper's Alg. 1
+                                            (PAPER.md:163-181): whole rows dealt to kappa partitions, one block each */
+    int32_t kappa;                       /* partitions of the Alg. 1 policy (0 under the default policy) */
+    int64_t max_partition_nnz[MTTKRP_MAX_MODES];   /* Alg. 1 policy: largest / smallest partition per mode, in nonzeros */
+    int64_t min_partition_nnz[MTTKRP_MAX_MODES];
+    int32_t fused_remap;                 /* 1: MTTKRP_FUSE=1 is in effect - the MTTKRP kernel of mode d also scatters the
+                                            records into the layout of mode (d+1)%N (Alg. 4 lines 15-19) */
+    int32_t reserved_;
 } mttkrp_info_t;
 
 /*

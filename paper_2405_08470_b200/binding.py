@@ -38,7 +38,10 @@ class Info(ctypes.Structure):
                 ("num_split_rows", ctypes.c_int64 * MAX_MODES), ("num_empty_rows", ctypes.c_int64 * MAX_MODES),
                 ("bytes_held", ctypes.c_int64), ("bytes_paper_format", ctypes.c_int64),
                 ("remaps_done", ctypes.c_int64), ("key_order", (ctypes.c_int32 * MAX_MODES) * MAX_MODES),
-                ("remap_blocked", ctypes.c_int32 * MAX_MODES), ("remap_avg_run", ctypes.c_double * MAX_MODES)]
+                ("remap_blocked", ctypes.c_int32 * MAX_MODES), ("remap_avg_run", ctypes.c_double * MAX_MODES),
+                ("shard_policy", ctypes.c_int32), ("kappa", ctypes.c_int32),
+                ("max_partition_nnz", ctypes.c_int64 * MAX_MODES), ("min_partition_nnz", ctypes.c_int64 * MAX_MODES),
+                ("fused_remap", ctypes.c_int32), ("reserved_", ctypes.c_int32)]
 
 
 class Timing(ctypes.Structure):
@@ -216,6 +219,8 @@ class Mttkrp:
             "remaps_done": raw.remaps_done,
             "key_order": [list(raw.key_order[d])[:n] for d in range(n)],
             "remap_blocked": list(raw.remap_blocked)[:n], "remap_avg_run": list(raw.remap_avg_run)[:n],
+            "shard_policy": "alg1" if raw.shard_policy else "equal", "kappa": raw.kappa, "fused_remap": bool(raw.fused_remap),
+            "max_partition_nnz": list(raw.max_partition_nnz)[:n], "min_partition_nnz": list(raw.min_partition_nnz)[:n],
         }
 
     def partition_rows(self, d: int, kappa: int):

@@ -7,7 +7,6 @@
 #include <cstring>
 #include <algorithm>
 #include <new>
-#include <queue>
 #include <utility>
 #include <vector>
 #include "common.cuh"
@@ -52,6 +51,16 @@ static int ceil_log2(int64_t x) {
 // not depend on the path.
 static mttkrp_status_t ensure_layout(mttkrp_handle_s* h, int d, cudaStream_t st) {
     if (h->cur == d) return MTTKRP_OK;
+    if (h->alt_layout == d) {                             // the fused kernel of the previous mode already wrote layout d
+        uint32_t* t = h->rec_cur;                         // swap(T_in, T_out), Alg. 5 line 12
+        h->rec_cur = h->rec_alt;
+        h->rec_alt = t;
+        h->cur = d;
+        h->alt_layout = -1;
+        h->remaps_done++;
+        return MTTKRP_OK;
+    }
+    h->alt_layout = -1;                                   // any other pass overwrites the other copy
     const int N = h->N, from = h->cur;
     const int steps = ((d - from) % N + N) % N;
     if (steps == 1 || h->nnz == 0) return launch_remap(h, from, d, nullptr, st);
@@ -89,7 +98,14 @@ static mttkrp_status_t order_end(mttkrp_handle_s* h, cudaStream_t st) {
 // order of Alg. 5 costs one), then the MTTKRP kernels.
 static mttkrp_status_t run_mode(mttkrp_handle_s* h, int d, const float* const* factors, int R, float* out, cudaStream_t st) {
     MK_TRY(ensure_layout(h, d, st));
-    return launch_mttkrp(h, d, factors, R, out, st);
+    MK_TRY(launch_mttkrp(h, d, factors, R, out, st));
+    if (h->fuse && h->nnz > 0) {                          // the kernel also scattered the records into layout d+1
+        const int to = (d + 1) % h->N;
+        TimedLaunch tl(h->timing, kClsRemap, st);
+        MK_TRY(launch_remap_padding(h, d, to, st));
+        h->alt_layout = to;
+    }
+    return MTTKRP_OK;
 }
 
 }  // namespace mk
@@ -108,7 +124,8 @@ mttkrp_status_t mttkrp_workspace_bytes(int nmodes, const int64_t* dims, int64_t 
     LayoutPlan lp;
     MK_TRY(plan_layouts(nmodes, dims, nnz, &lp));
     WorkspacePlan p;
-    MK_TRY(plan_workspace(nmodes, dims, nnz, max_rank, lp.rec_words, device_sm_count(), &p));
+    const int sms = device_sm_count();
+    MK_TRY(plan_workspace(nmodes, dims, nnz, max_rank, lp.rec_words, sms, lp.policy ? (lp.kappa ? lp.kappa : sms) : 0, lp.fuse, &p));
     *bytes = p.total;
     return MTTKRP_OK;
 }
@@ -128,7 +145,8 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
     MK_TRY(plan_layouts(nmodes, dims, nnz, &lp));
     WorkspacePlan p;
     const int num_sms = device_sm_count();
-    MK_TRY(plan_workspace(nmodes, dims, nnz, max_rank, lp.rec_words, num_sms, &p));
+    const int kappa = lp.policy ? (lp.kappa ? lp.kappa : num_sms) : 0;
+    MK_TRY(plan_workspace(nmodes, dims, nnz, max_rank, lp.rec_words, num_sms, kappa, lp.fuse, &p));
     if (workspace_bytes < p.total) {
         set_error("workspace %zu bytes < required %zu", workspace_bytes, p.total);
         return MTTKRP_EWORKSPACE;
@@ -147,6 +165,10 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
     h->packed = lp.packed;
     h->shard_nnz = p.shard_nnz;
     h->num_shards = p.num_shards;
+    h->policy = lp.policy;
+    h->kappa = kappa;
+    h->fuse = lp.fuse;
+    h->alt_layout = -1;
     h->rec_cur = reinterpret_cast<uint32_t*>(ws + p.rec_a);
     h->rec_alt = reinterpret_cast<uint32_t*>(ws + p.rec_b);
     h->perm0 = reinterpret_cast<uint32_t*>(ws + p.perm0);
@@ -180,6 +202,9 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
         mm.lflags = reinterpret_cast<uint8_t*>(ws + p.lflags[d]);
         mm.empty_rows = reinterpret_cast<uint32_t*>(ws + p.empty[d]);
         mm.chains = reinterpret_cast<uint32_t*>(ws + p.chains[d]);
+        mm.bins = reinterpret_cast<uint32_t*>(ws + p.bins[d]);
+        mm.scat = reinterpret_cast<uint32_t*>(ws + p.scat[d]);
+        mm.sflags = reinterpret_cast<uint8_t*>(ws + p.sflags[d]);
         if (max_rank > 0) {
             h->stage_fac[d] = reinterpret_cast<float*>(ws + p.stage_fac[d]);
             h->stage_out[d] = reinterpret_cast<float*>(ws + p.stage_out[d]);
@@ -355,6 +380,10 @@ mttkrp_status_t mttkrp_get_info(mttkrp_handle_t h, mttkrp_info_t* info) {
     info->bytes_held = h->bytes_held;
     info->bytes_paper_format = (h->nnz * bits + 7) / 8;
     info->remaps_done = h->remaps_done;
+    info->fused_remap = h->fuse;
+    info->shard_policy = h->policy;
+    info->kappa = h->kappa;
+    for (int m = 0; m < h->N; ++m) { info->max_partition_nnz[m] = h->mode[m].max_bin; info->min_partition_nnz[m] = h->mode[m].min_bin; }
     return MTTKRP_OK;
 }
 
@@ -397,27 +426,11 @@ mttkrp_status_t mttkrp_partition_rows(mttkrp_handle_t h, int d, int kappa, int32
     MK_TRY(launch_row_degrees(h, d, deg_dev, st));
     MK_TRY(order_end(h, st));
     const int64_t rows = h->dims[d];
-    try {                                                      // std::vector / stable_sort may throw: nothing crosses the C ABI
-    std::vector<int32_t> deg((size_t)rows);
+    std::vector<int32_t> deg;
+    try { deg.resize((size_t)rows); } catch (...) { set_error("mttkrp_partition_rows: out of host memory"); return MTTKRP_EINVAL; }
     MK_CUDA(cudaMemcpyAsync(deg.data(), deg_dev, sizeof(int32_t) * (size_t)rows, cudaMemcpyDeviceToHost, st));
     MK_CUDA(cudaStreamSynchronize(st));
-    // Alg. 1: vertices by descending degree, each to the least-loaded partition.
-    std::vector<int32_t> order((size_t)rows);
-    for (int64_t i = 0; i < rows; ++i) order[(size_t)i] = (int32_t)i;
-    std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) { return deg[(size_t)a] > deg[(size_t)b]; });
-    typedef std::pair<int64_t, int> Bin;                       // (load, partition id): min-heap, ties to the lowest id
-    std::priority_queue<Bin, std::vector<Bin>, std::greater<Bin>> heap;
-    for (int z = 0; z < kappa; ++z) { loads[z] = 0; heap.push(Bin(0, z)); }
-    for (int64_t q = 0; q < rows; ++q) {
-        const int32_t v = order[(size_t)q];
-        Bin b = heap.top();
-        heap.pop();
-        b.first += deg[(size_t)v];
-        loads[b.second] = b.first;
-        if (part_of_row) part_of_row[v] = b.second;
-        heap.push(b);
-    }
-    } catch (...) {
+    if (!lpt_partition(deg.data(), rows, kappa, part_of_row, loads)) {
         set_error("mttkrp_partition_rows: out of host memory");
         return MTTKRP_EINVAL;
     }

@@ -7,6 +7,11 @@
 #include <cstdlib>
 #include <cstring>
 #include <algorithm>
+#include <functional>
+#include <new>
+#include <queue>
+#include <utility>
+#include <vector>
 #include "common.cuh"
 
 namespace mk {
@@ -41,7 +46,7 @@ static int choose_shard_nnz(int64_t nnz, int num_sms) {
 }
 
 mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_rank, int rec_words, int num_sms,
-                               WorkspacePlan* p) {
+                               int kappa, int fuse, WorkspacePlan* p) {
     memset(p, 0, sizeof(*p));
     const size_t n = (size_t)nnz;
     p->shard_nnz = choose_shard_nnz(nnz, num_sms);
@@ -60,6 +65,9 @@ mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_
     p->jump[1] = off; if (N >= 4) off = align_up(off + 4 * n);
     for (int d = 0; d < N; ++d) { p->empty[d] = off; off = align_up(off + 4 * (size_t)dims[d]); }
     for (int d = 0; d < N; ++d) { p->chains[d] = off; off = align_up(off + 12 * (size_t)p->num_shards); }
+    for (int d = 0; d < N; ++d) { p->bins[d] = off; if (kappa > 0) off = align_up(off + 4 * ((size_t)kappa + 1)); }
+    for (int d = 0; d < N; ++d) { p->scat[d] = off; if (fuse) off = align_up(off + 4 * n); }
+    for (int d = 0; d < N; ++d) { p->sflags[d] = off; if (fuse) off = align_up(off + n); }
     p->carry = off; off = align_up(off + (size_t)2 * p->num_shards * kMaxRank * 4);
     if (max_rank > 0) {
         for (int d = 0; d < N; ++d) { p->stage_fac[d] = off; off = align_up(off + (size_t)dims[d] * max_rank * 4); }
@@ -92,6 +100,12 @@ __global__ void k_validate(const int32_t* __restrict__ idx, int64_t nnz, int N, 
         int32_t v = idx[(size_t)m * nnz + k];
         if (v < 0 || (int64_t)v >= dims_dev[m]) atomicOr(bad, 1u << m);
     }
+}
+
+// deg[key[k]] += 1 (Alg. 1's vertex degrees; create time only, global atomics are fine here)
+__global__ void k_count_keys(const uint32_t* __restrict__ key, int64_t n, uint32_t* __restrict__ deg) {
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) atomicAdd(deg + key[k], 1u);
 }
 
 __global__ void k_iota(uint32_t* __restrict__ p, int64_t n) {
@@ -338,6 +352,12 @@ __global__ void k_build_records_pk(const int32_t* __restrict__ idx, const float*
     rec[k] = pk_pack<N>(key, flags[k], k < nnz ? __float_as_uint(vals[src]) : 0u, pd);
 }
 
+// out[k] = table[idx[k]] for byte tables
+__global__ void k_gather_u8(const uint8_t* __restrict__ table, const uint32_t* __restrict__ idx, uint8_t* __restrict__ out, int64_t n) {
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) out[k] = table[idx[k]];
+}
+
 // key[j] = map[j] >> shift (the source block of destination position j)
 __global__ void k_block_keys(const uint32_t* __restrict__ map, int shift, uint32_t* __restrict__ key, int64_t n) {
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -403,6 +423,29 @@ __global__ void k_chain_fill(const uint32_t* __restrict__ kd, int64_t nnz, int S
     c[0] = (uint32_t)s;
     c[1] = (uint32_t)((lo - 1) / S);
     c[2] = r;
+}
+
+bool lpt_partition(const int32_t* deg, int64_t rows, int kappa, int32_t* part_of_row, int64_t* loads) {
+    try {
+        std::vector<int32_t> order((size_t)rows);
+        for (int64_t i = 0; i < rows; ++i) order[(size_t)i] = (int32_t)i;
+        std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) { return deg[a] > deg[b]; });
+        typedef std::pair<int64_t, int> Bin;                   // (load, partition id): min-heap, ties to the lowest id
+        std::priority_queue<Bin, std::vector<Bin>, std::greater<Bin>> heap;
+        for (int z = 0; z < kappa; ++z) { loads[z] = 0; heap.push(Bin(0, z)); }
+        for (int64_t q = 0; q < rows; ++q) {
+            const int32_t v = order[(size_t)q];
+            Bin b = heap.top();
+            heap.pop();
+            b.first += deg[v];
+            loads[b.second] = b.first;
+            if (part_of_row) part_of_row[v] = b.second;
+            heap.push(b);
+        }
+    } catch (...) {
+        return false;
+    }
+    return true;
 }
 
 static inline unsigned grid_for(int64_t n, int threads) { return (unsigned)std::max<int64_t>(1, (n + threads - 1) / threads); }
@@ -476,6 +519,17 @@ mttkrp_status_t plan_layouts(int N, const int64_t* dims, int64_t nnz, LayoutPlan
     }
     lp->packed = packed ? 1 : 0;
     lp->rec_words = packed ? 4 : N + 1;
+    const char* pol = getenv("MTTKRP_SHARD_POLICY");              // equal (default) | alg1 (the paper's partitioner)
+    if (pol && strcmp(pol, "equal") != 0 && strcmp(pol, "alg1") != 0) {
+        set_error("MTTKRP_SHARD_POLICY=%s is not one of equal, alg1", pol);
+        return MTTKRP_EINVAL;
+    }
+    lp->policy = (pol && strcmp(pol, "alg1") == 0) ? 1 : 0;
+    const char* fuse = getenv("MTTKRP_FUSE");                     // 1: Alg. 3 runs inside the MTTKRP kernel (16-byte records)
+    lp->fuse = (fuse && fuse[0] == '1' && lp->rec_words == 4 && lp->policy == 0) ? 1 : 0;
+    const char* kap = getenv("MTTKRP_KAPPA");
+    lp->kappa = kap ? atoi(kap) : 0;
+    if (lp->kappa < 0 || lp->kappa > 65536) { set_error("MTTKRP_KAPPA=%s outside [1, 65536]", kap); return MTTKRP_EINVAL; }
     return MTTKRP_OK;
 }
 
@@ -501,7 +555,6 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
     const size_t flag_n = (size_t)std::max<int64_t>(maxdim, nshards) + 1;
     uint32_t* flags = (uint32_t*)take(4 * flag_n);
     uint32_t* flags2 = (uint32_t*)take(4 * flag_n);
-    (void)flags2;
     uint32_t* sums = (uint32_t*)take(4 * (std::max<size_t>(256 * (size_t)nblocks + 1, (size_t)maxdim + 1) / kScanTile + 2));
     uint32_t* small = (uint32_t*)take(4096);          // [0]=bad flag, [8..8+2N) counts, then dims
     int64_t* dims_dev = (int64_t*)(small + 64);
@@ -540,6 +593,46 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
                     std::swap(ka, kb);
                     std::swap(pa, pb);
                 }
+                MK_CUDA(cudaGetLastError());
+            }
+            if (h->policy == 1) {
+                // Alg. 1 policy: the partition of the output row becomes the leading sort key ("order the
+                // hyperedges by partition id").  Degrees on the device, longest-first dealing on the host (as the paper
+                // preprocesses on the CPU), then the radix passes over the partition id.
+                const int64_t rows = h->dims[d];
+                const uint32_t* col = (const uint32_t*)idx + (size_t)d * n;
+                MK_CUDA(cudaMemsetAsync(flags, 0, 4 * (size_t)rows, st));
+                k_count_keys<<<grid_for(nnz, 256), 256, 0, st>>>(col, nnz, flags);
+                std::vector<int32_t> deg, part;
+                std::vector<int64_t> loads;
+                try { deg.resize((size_t)rows); part.resize((size_t)rows); loads.resize((size_t)h->kappa); }
+                catch (...) { set_error("out of host memory"); return MTTKRP_EINVAL; }
+                MK_CUDA(cudaMemcpyAsync(deg.data(), flags, 4 * (size_t)rows, cudaMemcpyDeviceToHost, st));
+                MK_CUDA(cudaStreamSynchronize(st));
+                if (!lpt_partition(deg.data(), rows, h->kappa, part.data(), loads.data())) { set_error("out of host memory"); return MTTKRP_EINVAL; }
+                std::vector<uint32_t> bins((size_t)h->kappa + 1);
+                bins[0] = 0;
+                mm.max_bin = 0;
+                mm.min_bin = nnz;
+                for (int z = 0; z < h->kappa; ++z) {
+                    bins[(size_t)z + 1] = bins[(size_t)z] + (uint32_t)loads[(size_t)z];
+                    mm.max_bin = std::max(mm.max_bin, loads[(size_t)z]);
+                    mm.min_bin = std::min(mm.min_bin, loads[(size_t)z]);
+                }
+                MK_CUDA(cudaMemcpyAsync(mm.bins, bins.data(), 4 * bins.size(), cudaMemcpyHostToDevice, st));
+                MK_CUDA(cudaMemcpyAsync(flags2, part.data(), 4 * (size_t)rows, cudaMemcpyHostToDevice, st));
+                k_gather_u32<<<grid_for(nnz, 256), 256, 0, st>>>(col, pa, ka, nnz);          // ka = i_d in the current order
+                k_apply_table<<<grid_for(nnz, 256), 256, 0, st>>>(flags2, ka, nnz);          // ka = partition of that row
+                const int pbits = ceil_log2_i64(h->kappa);
+                for (int shift = 0; shift < pbits; shift += 8) {
+                    k_radix_hist<<<(unsigned)nblocks, kSortThreads, 0, st>>>(ka, nnz, shift, hist, nblocks);
+                    MK_TRY(exclusive_scan(hist, 256 * nblocks, sums, st));
+                    k_radix_scatter<<<(unsigned)nblocks, kSortThreads, 0, st>>>(ka, pa, kb, pb, nnz, shift, hist, nblocks);
+                    std::swap(ka, kb);
+                    std::swap(pa, pb);
+                }
+                k_gather_u32<<<grid_for(nnz, 256), 256, 0, st>>>(col, pa, ka, nnz);          // ka = i_d in mode-d order again
+                MK_CUDA(cudaStreamSynchronize(st));                                            // the host vectors go out of scope
                 MK_CUDA(cudaGetLastError());
             }
             // pa = perm_d, ka = idx[d] in mode-d order
@@ -606,6 +699,14 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
             k_invert<<<grid_for(nnz, 256), 256, 0, st>>>(h->mode[d].next, inv, nnz);
             k_gather_u32<<<grid_for(nnz, 256), 256, 0, st>>>(inv, perm_e, h->mode[d].next, nnz);
         }
+        if (h->fuse) {
+            // Scatter form of every transition for the fused kernel (Alg. 3 as written): scat_d = next_d^-1
+            // is the remap id of mode (d+1)%N, sflags_d the next layout's run-end flags read through it.
+            for (int d = 0; d < N; ++d) {
+                k_invert<<<grid_for(nnz, 256), 256, 0, st>>>(h->mode[d].next, h->mode[d].scat, nnz);
+                k_gather_u8<<<grid_for(nnz, 256), 256, 0, st>>>(h->mode[(d + 1) % N].lflags, h->mode[d].scat, h->mode[d].sflags, nnz);
+            }
+        }
         MK_CUDA(cudaGetLastError());
         // Blocked remap order (remap.cu): destination positions of the remap d -> d+1 grouped, stably,
         // by the source block they read from: one 8-bit radix pass on the block id.  The block is sized
@@ -639,7 +740,7 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
     MK_CUDA(cudaStreamSynchronize(st));
     const char* benv = getenv("MTTKRP_REMAP_BLOCKED");           // 0 / 1 force the choice (experiments)
     for (int d = 0; d < N; ++d) {
-        h->mode[d].n_chains = nnz > 0 ? counts[2 * d] : 0;
+        h->mode[d].n_chains = (nnz > 0 && h->policy == 0) ? counts[2 * d] : 0;   // Alg. 1 policy: no row spans blocks
         h->mode[d].n_empty = nnz > 0 ? counts[2 * d + 1] : h->dims[d];
         // Use the blocked order when the source window fits L2 comfortably, the destination runs are
         // long enough to store whole sectors (average run >= 4 records), and the plain walk is a random

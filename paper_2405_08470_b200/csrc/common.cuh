@@ -71,6 +71,25 @@ __device__ __forceinline__ uint4 pk_pack(const uint32_t* k, uint32_t flags, uint
     return make_uint4((uint32_t)w01, (uint32_t)(w01 >> 32), k[N - 1], val);
 }
 
+// Field permutation of a remap pass: the key at level l of the destination layout is the key at level src[l] of
+// the source layout.  RemapPk says where that source key sits in a packed record.
+struct FieldMap { int src[kMaxModes]; };
+struct RemapPk {
+    int32_t soff[kMaxModes];      // bit offset of the source field in (w1:w0), or -1: it is w2 (the last key)
+    uint32_t smask[kMaxModes];
+};
+// What the MTTKRP kernel needs to run Alg. 3 itself (Alg. 4 lines 15-19; MTTKRP_FUSE=1):
+// T_out[scat[pos]] = the record at position pos, re-ordered for the next mode's layout.
+struct FuseArgs {
+    uint32_t* out_rec;            // T_out
+    const uint32_t* scat;         // [nnz] remap id for mode (d+1) mod N: position in the next layout
+    const uint8_t* sflags;        // [nnz] run-end flags of the next layout at that position
+    int64_t nnz;                  // records beyond nnz are padding and are not scattered
+    FieldMap fm;
+    RemapPk rp;
+    PackDesc dd;                  // packed records: bit layout of the next layout
+};
+
 // Per-mode tables built by mttkrp_create.
 struct ModeMeta {
     int order[kMaxModes];     // sort-key order of this layout, order[0] == mode
@@ -91,6 +110,10 @@ struct ModeMeta {
     int64_t n_empty;
     uint32_t* chains;         // [n_chains][3] = {first shard, last shard, row} for rows spanning shards
     int64_t n_chains;
+    uint32_t* scat;           // MTTKRP_FUSE: [nnz] inverse of `next` (scatter form of the remap d -> (d+1)%N)
+    uint8_t* sflags;          // MTTKRP_FUSE: [nnz] lflags of layout (d+1)%N read through scat
+    uint32_t* bins;           // Alg. 1 policy: [kappa+1] first position of every partition in this layout
+    int64_t max_bin, min_bin; // ... largest / smallest partition, in nonzeros
 };
 
 }  // namespace mk
@@ -128,6 +151,10 @@ struct mttkrp_handle_s {
     int packed;               // 1: 16-byte packed records (N >= 4 and the index widths fit, see PackDesc)
     int shard_nnz;
     int64_t num_shards;
+    int fuse;                 // MTTKRP_FUSE=1: the MTTKRP kernel of mode d also writes the tensor copy of layout (d+1)%N
+    int alt_layout;           // layout the OTHER tensor copy (rec_alt) holds completely, or -1
+    int policy;               // 0: equal-nnz shards (default), 1: the paper's Alg. 1 (whole rows dealt to kappa partitions)
+    int kappa;                // number of partitions of the Alg. 1 policy
     uint32_t* rec_cur;        // resident tensor copy T_in, layout `cur`
     uint32_t* rec_alt;        // T_out
     uint32_t* perm0;          // [nnz] original COO position of element k of layout 0
@@ -159,7 +186,7 @@ namespace mk {
 // ---- build.cu -------------------------------------------------------------------------------
 struct WorkspacePlan {
     size_t rec_a, rec_b, perm0, carry, jump[2];
-    size_t next[kMaxModes], empty[kMaxModes], chains[kMaxModes], ord[kMaxModes], osrc[kMaxModes], lflags[kMaxModes];
+    size_t next[kMaxModes], empty[kMaxModes], chains[kMaxModes], ord[kMaxModes], osrc[kMaxModes], lflags[kMaxModes], bins[kMaxModes], scat[kMaxModes], sflags[kMaxModes];
     size_t stage_fac[kMaxModes], stage_out[kMaxModes];
     size_t persistent_end;
     size_t scratch;          // start of the create-time scratch (may overlap rec_b)
@@ -173,15 +200,24 @@ struct LayoutPlan {
     PackDesc pk[kMaxModes];
     int packed;
     int rec_words;
+    int fuse;                // MTTKRP_FUSE=1 and 16-byte records and the default shard policy
+    int policy;              // MTTKRP_SHARD_POLICY: 0 equal (default), 1 alg1
+    int kappa;               // MTTKRP_KAPPA (alg1): 0 = one partition per SM
 };
 mttkrp_status_t plan_layouts(int N, const int64_t* dims, int64_t nnz, LayoutPlan* lp);   // EINVAL: bad MTTKRP_* override
-mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_rank, int rec_words, int num_sms, WorkspacePlan* p);
+mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_rank, int rec_words, int num_sms, int kappa,
+                               int fuse, WorkspacePlan* p);
+// Alg. 1 (reading 3): rows by descending degree (ties: lower index), each to the least-loaded
+// of kappa partitions (ties: lowest id).  Host code; returns false when out of memory.
+bool lpt_partition(const int32_t* deg, int64_t rows, int kappa, int32_t* part_of_row, int64_t* loads);
 int device_sm_count();       // SM count of the current device (148 when no device can be queried)
 mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char* ws,
                              const int32_t* idx, const float* vals, cudaStream_t st);
 
 // ---- remap.cu -------------------------------------------------------------------------------
 mttkrp_status_t launch_remap(mttkrp_handle_s* h, int from, int to, const uint32_t* jump, cudaStream_t st);   // swaps copies
+void remap_fields(const mttkrp_handle_s* h, int from, int to, FieldMap* fm, RemapPk* rp);
+mttkrp_status_t launch_remap_padding(mttkrp_handle_s* h, int from, int to, cudaStream_t st);   // padding records of rec_alt only
 mttkrp_status_t launch_export(const mttkrp_handle_s* h, int32_t* idx, float* vals, cudaStream_t st);
 mttkrp_status_t launch_row_degrees(const mttkrp_handle_s* h, int d, int32_t* deg_dev, cudaStream_t st);
 mttkrp_status_t launch_perm_step(const uint32_t* map, const uint32_t* in, uint32_t* out, int64_t nnz, cudaStream_t st);

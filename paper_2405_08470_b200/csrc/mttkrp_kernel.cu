@@ -188,7 +188,7 @@ struct Geo {
     static constexpr int ENT_WORDS = 2 * NPW * R;                       // per warp: first/last partial rows
     static constexpr int WARP_WORDS = RING_WORDS > ENT_WORDS ? RING_WORDS : ENT_WORDS;
     static constexpr int NL = N - 1;                     // accumulator levels t[0..NL-1]
-    static constexpr int MINB_DEF = N <= 3 ? (DEEP ? 3 : 5) : (N == 4 ? 4 : (N <= 6 ? 3 : 2));
+    static constexpr int MINB_DEF = N <= 3 ? (DEEP ? 3 : 5) : (N == 4 ? (PACKED ? 4 : 3) : (N == 5 ? 3 : 2));   // no instantiation spills
     static constexpr int MINB = DEEP ? (MK_MINB_DEEP ? MK_MINB_DEEP : MINB_DEF) : (MK_MINB ? MK_MINB : MINB_DEF);
     static constexpr int SMEM_BYTES = 4 * (WARPS * WARP_WORDS + WARPS * NPW * R + 2 * WARPS * R + WARPS * 2 * NPW + 2 * WARPS);
 };
@@ -220,8 +220,19 @@ __device__ __forceinline__ void merge_runs(const int* rows, const float* vecs, i
     if (cur_row >= 0) emit(cur_row, acc, run == 0, true);
 }
 
-template <int N, int R, bool DEEP, bool PACKED>
-__global__ void __launch_bounds__(kBlockThreads, Geo<N, R, DEEP, PACKED>::MINB) k_mttkrp(const KernelArgs<N> a) {
+// One piece of the mode-d layout, processed by one thread block: `count` records starting at position s_begin.
+//   BINS == false (default policy, equal-nnz shards): count == shard_nnz, `fast` is true; rows shared with the
+//     neighbouring shards leave their partials in the carry buffer (k_fixup sums them).
+//   BINS == true (the paper's Alg. 1 policy: whole output rows dealt to kappa partitions, one
+//     thread block per partition, k_mttkrp_bins): the block calls this for the consecutive pieces of its
+//     partition [.., seg_end); a row that continues into the next piece is carried in shared memory by the same
+//     block, so there is neither a carry buffer nor a fix-up pass.  The ragged last piece (count < shard_nnz,
+//     `fast` false) is walked with a plain loop.
+//   FUSE == true (MTTKRP_FUSE=1, 16-byte records): the block also executes Alg. 3 for its records, as the paper's
+//     kernel does (Alg. 4 lines 15-19): T_out[remap id for mode (d+1) mod N] = record.
+template <int N, int R, bool DEEP, bool PACKED, bool BINS, bool FUSE>
+__device__ __forceinline__ void shard_body(const KernelArgs<N>& a, const int64_t s_begin, const int count, const bool fast,
+                                           const int64_t seg_end, const FuseArgs& fa) {
     using Ge = Geo<N, R, DEEP, PACKED>;
     constexpr int V = Ge::V, LPN = Ge::LPN, NPW = Ge::NPW, WARPS = Ge::WARPS, G = Ge::G, K = Ge::K, D = Ge::D;
     constexpr int STAGES = Ge::STAGES, RECW = Ge::RECW, SLOTW = Ge::SLOTW, NL = Ge::NL;
@@ -242,17 +253,18 @@ __global__ void __launch_bounds__(kBlockThreads, Geo<N, R, DEEP, PACKED>::MINB) 
     float (*s_wvec)[R] = reinterpret_cast<float (*)[R]>(&s_first[WARPS][0][0]);
     int (*s_erow)[2 * NPW] = reinterpret_cast<int (*)[2 * NPW]>(&s_wvec[2 * WARPS][0]);
     int* s_wrow = &s_erow[WARPS][0];
+    float* const s_open = reinterpret_cast<float*>(&s_wrow[2 * WARPS]);  // BINS: the row carried into the next piece
+    int* const s_open_row = reinterpret_cast<int*>(s_open + R);
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int g = lane / LPN, sub = lane % LPN;
-    const int64_t shard = blockIdx.x;
-    // The record array is padded to a whole number of shards (value 0, keys of the last nonzero),
-    // so every chunk holds exactly C records and the loop needs no bounds checks.
-    const int64_t s_begin = shard * (int64_t)a.shard_nnz;
-    const int64_t s_end = s_begin + a.shard_nnz;
-    const int C = a.shard_nnz / G;                        // records per group; a multiple of K, > D
+    // Default policy: the record array is padded to a whole number of shards (value 0, keys of the last nonzero),
+    // so every chunk holds exactly C records and the fast loop needs no bounds checks.
+    const int64_t s_end = s_begin + count;
+    const int C = fast ? a.shard_nnz / G : (count + G - 1) / G;          // records per group; fast: a multiple of K, > D
     const int nrounds = C / K;
-    const int64_t cb = s_begin + (int64_t)(warp * NPW + g) * C;         // this group's first position
+    const int64_t cb = s_begin + min((int64_t)(warp * NPW + g) * C, (int64_t)count);         // this group's first position
+    const int64_t ce = s_begin + min((int64_t)(warp * NPW + g + 1) * C, (int64_t)count);     // one past its last
     const uint32_t* const grec = a.rec + (size_t)cb * RECW;
 
     uint32_t* const ring = &s_warp[warp][0];
@@ -331,202 +343,269 @@ __global__ void __launch_bounds__(kBlockThreads, Geo<N, R, DEEP, PACKED>::MINB) 
         t[0] = vzero();
     };
     constexpr bool BATCH = DEEP && N <= 3 && K == 8 && !PACKED;
-    if constexpr (BATCH) {
-        // ---- batch variant (N <= 3) -------------------------------------------------------------------------
-        // ptxas tracks every factor-row LDG of this loop on ONE scoreboard, so any wait drains all gathers in
-        // flight: a software pipeline degenerates into "issue, wait for everything, compute"
-        // (profiles/r2_scoreboards.md).  This variant makes that structure explicit and deep: the records of B = 4
-        // steps are read with back-to-back LDS.128, their B last-level rows and up to B fiber rows are requested
-        // together (up to 8 independent 128-bit gathers per lane in flight), then the B steps are computed.  Costs
-        // 64 registers (4 blocks per SM); one vote per batch replaces the per-step output-row-end test.
-        constexpr int B = 4;
-        Vec al[B], rb[B];
-        float val[B];
-        bool e1[B];
-        uint32_t anyend = 0;                              // OR of the batch's word 0: sign set = some output row ends in it
-        auto P = [&](uint32_t base) {                     // `base` = ring byte address of the batch's first record
-            uint4 q[B];
+    uint32_t lw[SLOTW];                                   // the chunk's last record
+    bool has = true;                                      // the group has at least one record (always, on the fast path)
+    if (!BINS || fast) {
+        if constexpr (BATCH) {
+            // ---- batch variant (N <= 3) -------------------------------------------------------------------------
+            // ptxas tracks every factor-row LDG of this loop on ONE scoreboard, so any wait drains all gathers in
+            // flight: a software pipeline degenerates into "issue, wait for everything, compute"
+            // (profiles/r2_scoreboards.md).  This variant makes that structure explicit and deep: the records of B = 4
+            // steps are read with back-to-back LDS.128, their B last-level rows and up to B fiber rows are requested
+            // together (up to 8 independent 128-bit gathers per lane in flight), then the B steps are computed.  Costs
+            // 64 registers (4 blocks per SM); one vote per batch replaces the per-step output-row-end test.
+            constexpr int B = 4;
+            Vec al[B], rb[B];
+            float val[B];
+            bool e1[B];
+            uint32_t anyend = 0;                              // OR of the batch's word 0: sign set = some output row ends in it
+            auto P = [&](uint32_t base) {                     // `base` = ring byte address of the batch's first record
+                uint4 q[B];
 #pragma unroll
-            for (int s = 0; s < B; ++s) q[s] = lds128(base + 4u * (uint32_t)(s * ROWW));
-            anyend = 0;
-#pragma unroll
-            for (int s = 0; s < B; ++s) {
-                if constexpr (N == 3) {
-                    al[s] = ld_row<LPN>(fb[2], q[s].z);
-                    e1[s] = (int32_t)q[s].y < 0;
-                    if (e1[s]) rb[s] = ld_row_flagged<LPN>(fiber_base, q[s].y, sub);
-                    val[s] = __uint_as_float(q[s].w);
-                } else {
-                    al[s] = ld_row<LPN>(fb[1], q[s].y);
-                    e1[s] = false;
-                    val[s] = __uint_as_float(q[s].z);
-                }
-                anyend |= q[s].x;
-            }
-        };
-        auto C = [&](uint32_t base) {
-            if (!__any_sync(0xffffffffu, (int32_t)anyend < 0)) {      // common: no output row ends in this batch
+                for (int s = 0; s < B; ++s) q[s] = lds128(base + 4u * (uint32_t)(s * ROWW));
+                anyend = 0;
 #pragma unroll
                 for (int s = 0; s < B; ++s) {
-                    vfmas(t[NL - 1], val[s], al[s]);
                     if constexpr (N == 3) {
-                        if (e1[s]) { vfma(t[0], rb[s], t[1]); t[1] = vzero(); }
+                        al[s] = ld_row<LPN>(fb[2], q[s].z);
+                        e1[s] = (int32_t)q[s].y < 0;
+                        if (e1[s]) rb[s] = ld_row_flagged<LPN>(fiber_base, q[s].y, sub);
+                        val[s] = __uint_as_float(q[s].w);
+                    } else {
+                        al[s] = ld_row<LPN>(fb[1], q[s].y);
+                        e1[s] = false;
+                        val[s] = __uint_as_float(q[s].z);
                     }
+                    anyend |= q[s].x;
                 }
-            } else {
+            };
+            auto C = [&](uint32_t base) {
+                if (!__any_sync(0xffffffffu, (int32_t)anyend < 0)) {      // common: no output row ends in this batch
 #pragma unroll
-                for (int s = 0; s < B; ++s) {
-                    vfmas(t[NL - 1], val[s], al[s]);
-                    if constexpr (N == 3) {
-                        if (e1[s]) { vfma(t[0], rb[s], t[1]); t[1] = vzero(); }
-                    }
-                    const uint32_t w0 = lds32(base + 4u * (uint32_t)(s * ROWW));
-                    if ((int32_t)w0 < 0) emit_row(w0 & kKeyMask);
-                }
-            }
-        };
-#pragma unroll
-        for (int r = 0; r < AHEAD; ++r) issue_round();
-        cp_async_wait<AHEAD - 1>();                       // round 0 has landed
-        __syncwarp();
-        P(ring_gs);
-        int stage = 0;
-        for (int r = 0; r < nrounds; ++r) {
-            issue_round();                                // round r+AHEAD, reuses the stage of round r-1
-            cp_async_wait<AHEAD - 1>();                   // rounds <= r+1 have landed
-            __syncwarp();
-            const int nstage = (stage + 1 == STAGES) ? 0 : stage + 1;
-            const uint32_t cs = ring_gs + 4u * (uint32_t)(stage * STAGEW);
-            const uint32_t ns = ring_gs + 4u * (uint32_t)(nstage * STAGEW);
-            C(cs);
-            P(cs + 4u * (uint32_t)(B * ROWW));
-            C(cs + 4u * (uint32_t)(B * ROWW));
-            if (r + 1 < nrounds) P(ns);
-            stage = nstage;
-            __syncwarp();                                 // everyone is done with round r's stage
-        }
-    } else {
-        Vec al[D];                                            // last-level rows for the D steps in flight
-        Vec rb[NL][D];                                        // rb[l][slot]: row of level l, gathered at the end of its run
-        float val[D];
-        bool e[NL][D];                                        // e[l][slot]: the run of level l ends at that step
-
-        // Issue the gathers of one step whose record sits at ring byte address `slot`.
-        auto prefetch = [&](uint32_t slot, int s) {
-            uint32_t w[SLOTW];
-#pragma unroll
-            for (int i = 0; i < SLOTW / 4; ++i) {
-                const uint4 v = lds128(slot + 16u * i);
-                w[4 * i] = v.x; w[4 * i + 1] = v.y; w[4 * i + 2] = v.z; w[4 * i + 3] = v.w;
-            }
-            if constexpr (PACKED) {                           // {w0, w1 = flags | keys, w2 = last key, val}
-                al[s] = ld_row<LPN>(fb[N - 1], w[2]);
-#pragma unroll
-                for (int l = 0; l < NL; ++l) e[l][s] = (w[1] & (0x80000000u >> l)) != 0;
-                if (__any_sync(0xffffffffu, e[NL - 1][s])) {
-#pragma unroll
-                    for (int l = 1; l < NL; ++l)
-                        if (e[l][s]) rb[l][s] = ld_row<LPN>(fb[l], pk_get(w[0], w[1], a.koff[l], a.kmask[l]));
-                }
-                val[s] = __uint_as_float(w[3]);
-            } else {
-                al[s] = ld_row<LPN>(fb[N - 1], w[N - 1]);
-#pragma unroll
-                for (int l = 0; l < NL; ++l) e[l][s] = (int32_t)w[l] < 0;
-                if constexpr (NL >= 2) {
-                    if (e[NL - 1][s]) rb[NL - 1][s] = ld_row_flagged<LPN>(fiber_base, w[NL - 1], sub);
-                }
-                if constexpr (NL >= 3) {                      // e_l implies e_{l+1}: one vote guards all upper levels
-                    if (__any_sync(0xffffffffu, e[NL - 2][s])) {
-#pragma unroll
-                        for (int l = 1; l < NL - 1; ++l)
-                            if (e[l][s]) rb[l][s] = ld_row_flagged<LPN>(a.fac[l], w[l], sub);
-                    }
-                }
-                val[s] = __uint_as_float(w[N]);
-            }
-        };
-        // Arithmetic of one step (its record sits at `slot`).
-        auto compute = [&](uint32_t slot, int s) {
-            vfmas(t[NL - 1], val[s], al[s]);
-            if constexpr (NL >= 2) {
-                if (e[NL - 1][s]) {
-                    vfma(t[NL - 2], rb[NL - 1][s], t[NL - 1]);
-                    t[NL - 1] = vzero();
-                }
-            }
-            if constexpr (NL >= 3) {
-                if (__any_sync(0xffffffffu, e[NL - 2][s])) {
-#pragma unroll
-                    for (int l = NL - 2; l >= 1; --l) {
-                        if (e[l][s]) {
-                            vfma(t[l - 1], rb[l][s], t[l]);
-                            t[l] = vzero();
+                    for (int s = 0; s < B; ++s) {
+                        vfmas(t[NL - 1], val[s], al[s]);
+                        if constexpr (N == 3) {
+                            if (e1[s]) { vfma(t[0], rb[s], t[1]); t[1] = vzero(); }
                         }
                     }
+                } else {
+#pragma unroll
+                    for (int s = 0; s < B; ++s) {
+                        vfmas(t[NL - 1], val[s], al[s]);
+                        if constexpr (N == 3) {
+                            if (e1[s]) { vfma(t[0], rb[s], t[1]); t[1] = vzero(); }
+                        }
+                        const uint32_t w0 = lds32(base + 4u * (uint32_t)(s * ROWW));
+                        if ((int32_t)w0 < 0) emit_row(w0 & kKeyMask);
+                    }
                 }
-            }
-            if (__any_sync(0xffffffffu, e[0][s])) {           // rare: an output row ends inside the chunk
-                // Every lane reads its group's row id first (a volatile load): the branch above then depends on the
-                // vote alone and stays warp-uniform; only the stores below are per lane.
-                uint32_t row;
-                if constexpr (PACKED) row = pk_get(lds32(slot), lds32(slot + 4), a.koff[0], a.kmask[0]);
-                else row = lds32(slot) & kKeyMask;
-                if (e[0][s]) emit_row(row);
-            }
-        };
-
-        // ---- prologue: rounds 0..AHEAD-1 in flight, round 0 landed ----------------------------------------
+            };
 #pragma unroll
-        for (int r = 0; r < AHEAD; ++r) issue_round();
-        cp_async_wait<AHEAD - 1>();                           // round 0 has landed
-        __syncwarp();
-#pragma unroll
-        for (int i = 0; i < D; ++i) prefetch(ring_gs + 4u * (uint32_t)(i * ROWW), i);
-        int stage = 0;                                        // r % STAGES
-        for (int r = 0; r < nrounds; ++r) {
-            issue_round();                                    // round r+AHEAD, reuses the stage of round r-1
-            cp_async_wait<AHEAD - 1>();                       // rounds <= r+1 have landed
+            for (int r = 0; r < AHEAD; ++r) issue_round();
+            cp_async_wait<AHEAD - 1>();                       // round 0 has landed
             __syncwarp();
-            const int nstage = (stage + 1 == STAGES) ? 0 : stage + 1;
-            const uint32_t cs = ring_gs + 4u * (uint32_t)(stage * STAGEW);            // this round's stage
-            const uint32_t ns = ring_gs + 4u * (uint32_t)(nstage * STAGEW);           // next round's stage
-            const bool more = r + 1 < nrounds;
-#pragma unroll
-            for (int i = 0; i < K; ++i) {
-                compute(cs + 4u * (uint32_t)(i * ROWW), i % D);
-                if (i + D < K) prefetch(cs + 4u * (uint32_t)((i + D) * ROWW), i % D);
-                else if (more) prefetch(ns + 4u * (uint32_t)((i + D - K) * ROWW), i % D);
+            P(ring_gs);
+            int stage = 0;
+            for (int r = 0; r < nrounds; ++r) {
+                issue_round();                                // round r+AHEAD, reuses the stage of round r-1
+                cp_async_wait<AHEAD - 1>();                   // rounds <= r+1 have landed
+                __syncwarp();
+                const int nstage = (stage + 1 == STAGES) ? 0 : stage + 1;
+                const uint32_t cs = ring_gs + 4u * (uint32_t)(stage * STAGEW);
+                const uint32_t ns = ring_gs + 4u * (uint32_t)(nstage * STAGEW);
+                C(cs);
+                P(cs + 4u * (uint32_t)(B * ROWW));
+                C(cs + 4u * (uint32_t)(B * ROWW));
+                if (r + 1 < nrounds) P(ns);
+                stage = nstage;
+                __syncwarp();                                 // everyone is done with round r's stage
             }
-            stage = nstage;
-            __syncwarp();                                     // everyone is done with round r's stage
+        } else {
+            Vec al[D];                                            // last-level rows for the D steps in flight
+            Vec rb[NL][D];                                        // rb[l][slot]: row of level l, gathered at the end of its run
+            float val[D];
+            bool e[NL][D];                                        // e[l][slot]: the run of level l ends at that step
+
+            // Issue the gathers of one step whose record sits at ring byte address `slot`.
+            auto prefetch = [&](uint32_t slot, int s) {
+                uint32_t w[SLOTW];
+#pragma unroll
+                for (int i = 0; i < SLOTW / 4; ++i) {
+                    const uint4 v = lds128(slot + 16u * i);
+                    w[4 * i] = v.x; w[4 * i + 1] = v.y; w[4 * i + 2] = v.z; w[4 * i + 3] = v.w;
+                }
+                if constexpr (PACKED) {                           // {w0, w1 = flags | keys, w2 = last key, val}
+                    al[s] = ld_row<LPN>(fb[N - 1], w[2]);
+#pragma unroll
+                    for (int l = 0; l < NL; ++l) e[l][s] = (w[1] & (0x80000000u >> l)) != 0;
+#pragma unroll
+                    for (int l = 1; l < NL; ++l)
+                        if (e[l][s]) rb[l][s] = ld_row_flagged<LPN>(a.fac[l], pk_get(w[0], w[1], a.koff[l], a.kmask[l]), sub);
+                    val[s] = __uint_as_float(w[3]);
+                } else {
+                    al[s] = ld_row<LPN>(fb[N - 1], w[N - 1]);
+#pragma unroll
+                    for (int l = 0; l < NL; ++l) e[l][s] = (int32_t)w[l] < 0;
+                    if constexpr (NL >= 2) {
+                        if (e[NL - 1][s]) rb[NL - 1][s] = ld_row_flagged<LPN>(fiber_base, w[NL - 1], sub);
+                    }
+#pragma unroll
+                    for (int l = 1; l < NL - 1; ++l)
+                        if (e[l][s]) rb[l][s] = ld_row_flagged<LPN>(a.fac[l], w[l], sub);
+                    val[s] = __uint_as_float(w[N]);
+                }
+            };
+            // Arithmetic of one step (its record sits at `slot`).
+            auto compute = [&](uint32_t slot, int s) {
+                vfmas(t[NL - 1], val[s], al[s]);
+                if constexpr (NL >= 2) {
+                    if (e[NL - 1][s]) {
+                        vfma(t[NL - 2], rb[NL - 1][s], t[NL - 1]);
+                        t[NL - 1] = vzero();
+                    }
+                }
+                // upper fiber levels: plain predication (a vote + branch per level takes the scheduler's freedom to hoist
+                // the gathers: measured 10-28 % slower for N = 4, 5)
+#pragma unroll
+                for (int l = NL - 2; l >= 1; --l) {
+                    if (e[l][s]) {
+                        vfma(t[l - 1], rb[l][s], t[l]);
+                        t[l] = vzero();
+                    }
+                }
+                if (__any_sync(0xffffffffu, e[0][s])) {           // rare: an output row ends inside the chunk
+                    // Every lane reads its group's row id first (a volatile load): the branch above then depends on the
+                    // vote alone and stays warp-uniform; only the stores below are per lane.
+                    uint32_t row;
+                    if constexpr (PACKED) row = pk_get(lds32(slot), lds32(slot + 4), a.koff[0], a.kmask[0]);
+                    else row = lds32(slot) & kKeyMask;
+                    if (e[0][s]) emit_row(row);
+                }
+            };
+
+            // Dynamic tensor remapping inside the compute kernel (FUSE): lane p % LPN moves record p of the round.  The
+            // remap id and the next layout's flags are fetched at the start of the round, the record is re-read from
+            // the ring after the round's arithmetic, re-ordered for the next layout and scattered (Alg. 3).
+            uint32_t f_dst[NPIECE], f_fl[NPIECE];
+            auto fuse_load = [&](int r) {
+#pragma unroll
+                for (int i = 0; i < NPIECE; ++i) {
+                    const int p = sub + i * LPN;
+                    const int64_t pos = cb + (int64_t)r * K + p;
+                    f_dst[i] = 0xffffffffu;
+                    if (p < K && pos < fa.nnz) { f_dst[i] = __ldg(fa.scat + pos); f_fl[i] = __ldg(fa.sflags + pos); }
+                }
+            };
+            auto fuse_store = [&](uint32_t cs) {
+#pragma unroll
+                for (int i = 0; i < NPIECE; ++i) {
+                    const int p = sub + i * LPN;
+                    if (p < K && f_dst[i] != 0xffffffffu) {
+                        const uint4 q = lds128(cs + 4u * (uint32_t)(p * ROWW));
+                        uint32_t k[N];
+                        uint4 o;
+                        if constexpr (PACKED) {
+#pragma unroll
+                            for (int l = 0; l < N; ++l)
+                                k[l] = fa.rp.soff[l] < 0 ? (q.z & fa.rp.smask[l]) : pk_get(q.x, q.y, fa.rp.soff[l], fa.rp.smask[l]);
+                            o = pk_pack<N>(k, f_fl[i], q.w, fa.dd);
+                        } else {
+                            const uint32_t f[3] = {q.x & kKeyMask, q.y & kKeyMask, q.z & kKeyMask};
+#pragma unroll
+                            for (int l = 0; l < 3; ++l) k[l] = fa.fm.src[l] == 0 ? f[0] : (fa.fm.src[l] == 1 ? f[1] : f[2]);
+                            apply_run_flags<3>(k, f_fl[i]);
+                            o = make_uint4(k[0], k[1], k[2], q.w);
+                        }
+                        *(reinterpret_cast<uint4*>(fa.out_rec) + f_dst[i]) = o;
+                    }
+                }
+            };
+
+            // ---- prologue: rounds 0..AHEAD-1 in flight, round 0 landed ----------------------------------------
+#pragma unroll
+            for (int r = 0; r < AHEAD; ++r) issue_round();
+            cp_async_wait<AHEAD - 1>();                           // round 0 has landed
+            __syncwarp();
+#pragma unroll
+            for (int i = 0; i < D; ++i) prefetch(ring_gs + 4u * (uint32_t)(i * ROWW), i);
+            int stage = 0;                                        // r % STAGES
+            for (int r = 0; r < nrounds; ++r) {
+                issue_round();                                    // round r+AHEAD, reuses the stage of round r-1
+                cp_async_wait<AHEAD - 1>();                       // rounds <= r+1 have landed
+                __syncwarp();
+                const int nstage = (stage + 1 == STAGES) ? 0 : stage + 1;
+                const uint32_t cs = ring_gs + 4u * (uint32_t)(stage * STAGEW);            // this round's stage
+                const uint32_t ns = ring_gs + 4u * (uint32_t)(nstage * STAGEW);           // next round's stage
+                const bool more = r + 1 < nrounds;
+                if constexpr (FUSE) fuse_load(r);
+#pragma unroll
+                for (int i = 0; i < K; ++i) {
+                    compute(cs + 4u * (uint32_t)(i * ROWW), i % D);
+                    if (i + D < K) prefetch(cs + 4u * (uint32_t)((i + D) * ROWW), i % D);
+                    else if (more) prefetch(ns + 4u * (uint32_t)((i + D - K) * ROWW), i % D);
+                }
+                if constexpr (FUSE) fuse_store(cs);
+                stage = nstage;
+                __syncwarp();                                     // everyone is done with round r's stage
+            }
+        }
+        cp_async_wait<0>();
+        __syncwarp();
+        const uint32_t* const last_rec = ring_g + ((nrounds - 1) % STAGES) * STAGEW + (K - 1) * ROWW;
+#pragma unroll
+        for (int i = 0; i < SLOTW; ++i) lw[i] = last_rec[i];
+    } else {
+        // ragged piece (BINS only): one record at a time straight from global memory, gathers not overlapped
+        has = ce > cb;
+        for (int64_t pos = cb; pos < ce; ++pos) {
+            const uint32_t* rp = a.rec + (size_t)pos * RECW;
+#pragma unroll
+            for (int i = 0; i < RECW; ++i) lw[i] = __ldg(rp + i);
+            uint32_t key[N];
+            bool en[NL];
+            float v;
+            if constexpr (PACKED) {
+#pragma unroll
+                for (int l = 0; l < NL; ++l) { key[l] = pk_get(lw[0], lw[1], a.koff[l], a.kmask[l]); en[l] = (lw[1] & (0x80000000u >> l)) != 0; }
+                key[N - 1] = lw[2];
+                v = __uint_as_float(lw[3]);
+            } else {
+#pragma unroll
+                for (int l = 0; l < NL; ++l) { key[l] = lw[l] & kKeyMask; en[l] = (int32_t)lw[l] < 0; }
+                key[N - 1] = lw[N - 1];
+                v = __uint_as_float(lw[N]);
+            }
+            vfmas(t[NL - 1], v, ld_row<LPN>(fb[N - 1], key[N - 1]));
+#pragma unroll
+            for (int l = NL - 1; l >= 1; --l) {
+                if (en[l]) { vfma(t[l - 1], ld_row<LPN>(fb[l], key[l]), t[l]); t[l] = vzero(); }
+            }
+            if (en[0]) emit_row(key[0]);
         }
     }
-    cp_async_wait<0>();
-    __syncwarp();
     // ---- chunk epilogue -----------------------------------------------------------------------------------
     // The chunk's last record leaves its inner runs open unless they end there: fold them now (the level's
     // row is the last record's key), so that t[0] holds everything the chunk contributes to its last row.
-    const uint32_t* const last_rec = ring_g + ((nrounds - 1) % STAGES) * STAGEW + (K - 1) * ROWW;
-    uint32_t lw[SLOTW];
+    if (has) {
 #pragma unroll
-    for (int i = 0; i < SLOTW; ++i) lw[i] = last_rec[i];
-#pragma unroll
-    for (int l = NL - 1; l >= 1; --l) {
-        bool ended;
-        uint32_t key;
-        if constexpr (PACKED) { ended = (lw[1] & (0x80000000u >> l)) != 0; key = pk_get(lw[0], lw[1], a.koff[l], a.kmask[l]); }
-        else { ended = (int32_t)lw[l] < 0; key = lw[l] & kKeyMask; }
-        if (!ended) {
-            const Vec row = ld_row<LPN>(fb[l], key);
-            vfma(t[l - 1], row, t[l]);
-            t[l] = vzero();
+        for (int l = NL - 1; l >= 1; --l) {
+            bool ended;
+            uint32_t key;
+            if constexpr (PACKED) { ended = (lw[1] & (0x80000000u >> l)) != 0; key = pk_get(lw[0], lw[1], a.koff[l], a.kmask[l]); }
+            else { ended = (int32_t)lw[l] < 0; key = lw[l] & kKeyMask; }
+            if (!ended) {
+                const Vec row = ld_row<LPN>(fb[l], key);
+                vfma(t[l - 1], row, t[l]);
+                t[l] = vzero();
+            }
         }
     }
-    bool last_open;                                       // the chunk's last output row continues past the chunk
-    uint32_t last_row;
-    if constexpr (PACKED) { last_open = (lw[1] & 0x80000000u) == 0; last_row = pk_get(lw[0], lw[1], a.koff[0], a.kmask[0]); }
-    else { last_open = (int32_t)lw[0] >= 0; last_row = lw[0] & kKeyMask; }
+    bool last_open = false;                               // the chunk's last output row continues past the chunk
+    uint32_t last_row = 0;
+    if (has) {
+        if constexpr (PACKED) { last_open = (lw[1] & 0x80000000u) == 0; last_row = pk_get(lw[0], lw[1], a.koff[0], a.kmask[0]); }
+        else { last_open = (int32_t)lw[0] >= 0; last_row = lw[0] & kKeyMask; }
+    }
     __syncwarp();
     // The still-open row goes to the first (nothing emitted yet) or last partial-row entry; a row that ended
     // exactly at the chunk's last record was already emitted by the loop.
@@ -536,7 +615,10 @@ __global__ void __launch_bounds__(kBlockThreads, Geo<N, R, DEEP, PACKED>::MINB) 
         vstore(dst, t[0]);
     }
     if (sub == 0) {
-        if (last_open) {
+        if (!has) {
+            s_erow[warp][2 * g] = -1;                     // ragged piece: this group got no record
+            s_erow[warp][2 * g + 1] = -1;
+        } else if (last_open) {
             s_erow[warp][2 * g + (first_done ? 1 : 0)] = (int)last_row;
             if (!first_done) s_erow[warp][2 * g + 1] = -1;
         } else {
@@ -586,29 +668,86 @@ __global__ void __launch_bounds__(kBlockThreads, Geo<N, R, DEEP, PACKED>::MINB) 
     }
     __syncthreads();
 
-    // level 2: merge the warps' partial rows; rows shared with a neighbouring shard go to the carry buffer
+    // level 2: merge the warps' partial rows
     if (warp == 0) {
         auto key0_at = [&](int64_t pos) {
             const uint32_t* p = a.rec + (size_t)pos * RECW;
             if constexpr (PACKED) return pk_get(__ldg(p), __ldg(p + 1), a.koff[0], a.kmask[0]);
             else return __ldg(p) & kKeyMask;                            // k_0 sits in word 0
         };
-        const uint32_t first_row = key0_at(s_begin);
-        const uint32_t end_row = key0_at(s_end - 1);
-        const bool head_shared = s_begin > 0 && key0_at(s_begin - 1) == first_row;
-        const bool tail_shared = s_end < a.nnz && key0_at(s_end) == end_row;
         constexpr int CPL = (R + 31) / 32;
-        merge_runs<R>(s_wrow, &s_wvec[0][0], 2 * WARPS, lane, [&](int row, const float* acc, bool, bool) {
-            float* dst;
-            if ((uint32_t)row == first_row && head_shared) dst = a.carry + (size_t)(2 * shard) * R;
-            else if ((uint32_t)row == end_row && tail_shared) dst = a.carry + (size_t)(2 * shard + 1) * R;
-            else dst = a.out + (size_t)row * R;
+        if constexpr (!BINS) {
+            // rows shared with a neighbouring shard go to the carry buffer (k_fixup sums them in fixed order)
+            const int64_t shard = s_begin / a.shard_nnz;
+            const uint32_t first_row = key0_at(s_begin);
+            const uint32_t end_row = key0_at(s_end - 1);
+            const bool head_shared = s_begin > 0 && key0_at(s_begin - 1) == first_row;
+            const bool tail_shared = s_end < a.nnz && key0_at(s_end) == end_row;
+            merge_runs<R>(s_wrow, &s_wvec[0][0], 2 * WARPS, lane, [&](int row, const float* acc, bool, bool) {
+                float* dst;
+                if ((uint32_t)row == first_row && head_shared) dst = a.carry + (size_t)(2 * shard) * R;
+                else if ((uint32_t)row == end_row && tail_shared) dst = a.carry + (size_t)(2 * shard + 1) * R;
+                else dst = a.out + (size_t)row * R;
 #pragma unroll
-            for (int q = 0; q < CPL; ++q) {
-                const int col = lane + 32 * q;
-                if (col < R) dst[col] = acc[q];
-            }
-        });
+                for (int q = 0; q < CPL; ++q) {
+                    const int col = lane + 32 * q;
+                    if (col < R) dst[col] = acc[q];
+                }
+            });
+        } else {
+            // Alg. 1 policy: the whole partition belongs to this block, so a row that continues into the block's
+            // next piece is carried in shared memory (s_open) and stored once, when it ends.
+            const bool more = s_end < seg_end;
+            const uint32_t next_row = more ? key0_at(s_end) : 0u;
+            const int open_row = *s_open_row;
+            __syncwarp();
+            merge_runs<R>(s_wrow, &s_wvec[0][0], 2 * WARPS, lane, [&](int row, const float* acc, bool, bool is_last) {
+                const bool cont_prev = row == open_row;
+                const bool cont_next = is_last && more && (uint32_t)row == next_row;
+#pragma unroll
+                for (int q = 0; q < CPL; ++q) {
+                    const int col = lane + 32 * q;
+                    if (col < R) {
+                        const float v = acc[q] + (cont_prev ? s_open[col] : 0.f);
+                        if (cont_next) s_open[col] = v;
+                        else a.out[(size_t)row * R + col] = v;
+                    }
+                }
+                if (lane == 0) {
+                    if (cont_next) *s_open_row = row;
+                    else if (cont_prev) *s_open_row = -1;
+                }
+            });
+        }
+    }
+}
+
+// Default policy: one thread block per equal-nnz shard.
+template <int N, int R, bool DEEP, bool PACKED>
+__global__ void __launch_bounds__(kBlockThreads, Geo<N, R, DEEP, PACKED>::MINB) k_mttkrp(const KernelArgs<N> a) {
+    shard_body<N, R, DEEP, PACKED, false, false>(a, (int64_t)blockIdx.x * a.shard_nnz, a.shard_nnz, true, 0, FuseArgs());
+}
+
+// Same, with the dynamic tensor remapping of Alg. 3 executed by the same kernel (MTTKRP_FUSE=1; 16-byte records).
+template <int N, int R, bool PACKED>
+__global__ void __launch_bounds__(kBlockThreads, Geo<N, R, false, PACKED>::MINB) k_mttkrp_fused(const KernelArgs<N> a, const FuseArgs fa) {
+    shard_body<N, R, false, PACKED, false, true>(a, (int64_t)blockIdx.x * a.shard_nnz, a.shard_nnz, true, 0, fa);
+}
+
+// The paper's Alg. 1 policy (Alg. 4/5: one thread block per partition B_{d,z}): block z walks the
+// records [bins[z], bins[z+1]) of the partition-ordered layout in pieces of shard_nnz and owns every output row in it.
+template <int N, int R, bool PACKED>
+__global__ void __launch_bounds__(kBlockThreads, Geo<N, R, false, PACKED>::MINB) k_mttkrp_bins(const KernelArgs<N> a,
+                                                                                               const uint32_t* __restrict__ bins) {
+    extern __shared__ uint4 smem_raw[];
+    int* const s_open_row = reinterpret_cast<int*>(reinterpret_cast<char*>(smem_raw) + Geo<N, R, false, PACKED>::SMEM_BYTES) + R;
+    if (threadIdx.x == 0) *s_open_row = -1;
+    __syncthreads();
+    const int64_t begin = bins[blockIdx.x], end = bins[blockIdx.x + 1];
+    for (int64_t p = begin; p < end; p += a.shard_nnz) {
+        const int count = (int)min((int64_t)a.shard_nnz, end - p);
+        shard_body<N, R, false, PACKED, true, false>(a, p, count, count == a.shard_nnz, end, FuseArgs());
+        __syncthreads();                                  // the next piece reuses the shared-memory areas
     }
 }
 
@@ -689,7 +828,39 @@ static mttkrp_status_t launch_nr(mttkrp_handle_s* h, int d, const float* const* 
             k_mttkrp<N, R, DEEP, PACKED><<<(unsigned)h->num_shards, kBlockThreads, smem, st>>>(a);
             return MTTKRP_OK;
         };
-        if constexpr (N <= 3) {
+        auto launch_bins = [&](auto packed_tag) -> mttkrp_status_t {
+            constexpr bool PACKED = decltype(packed_tag)::value;
+            constexpr int smem = Geo<N, R, false, PACKED>::SMEM_BYTES + 4 * (R + 4);      // + the carried row
+            if constexpr (smem > 48 * 1024)
+                MK_CUDA(cudaFuncSetAttribute(k_mttkrp_bins<N, R, PACKED>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            TimedLaunch tl(h->timing, kClsMttkrp, st);
+            k_mttkrp_bins<N, R, PACKED><<<(unsigned)h->kappa, kBlockThreads, smem, st>>>(a, mm.bins);
+            return MTTKRP_OK;
+        };
+        auto launch_fused = [&](auto packed_tag) -> mttkrp_status_t {
+            constexpr bool PACKED = decltype(packed_tag)::value;
+            constexpr int smem = Geo<N, R, false, PACKED>::SMEM_BYTES;
+            FuseArgs fa;
+            const int to = (d + 1) % N;
+            fa.out_rec = h->rec_alt;
+            fa.scat = mm.scat;
+            fa.sflags = mm.sflags;
+            fa.nnz = h->nnz;
+            remap_fields(h, d, to, &fa.fm, &fa.rp);
+            fa.dd = h->mode[to].pk;
+            if constexpr (smem > 48 * 1024)
+                MK_CUDA(cudaFuncSetAttribute(k_mttkrp_fused<N, R, PACKED>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            TimedLaunch tl(h->timing, kClsMttkrp, st);
+            k_mttkrp_fused<N, R, PACKED><<<(unsigned)h->num_shards, kBlockThreads, smem, st>>>(a, fa);
+            return MTTKRP_OK;
+        };
+        if (h->fuse) {                                    // remap inside the compute kernel (Alg. 4 lines 15-19)
+            if constexpr (N == 3) MK_TRY(launch_fused(std::false_type{}));
+            else if constexpr (N >= 4) { if (h->packed) MK_TRY(launch_fused(std::true_type{})); }
+        } else if (h->policy == 1) {                      // the paper's Alg. 1 policy: one block per partition, no fix-up
+            if (h->packed) { if constexpr (N >= 4) MK_TRY(launch_bins(std::true_type{})); }
+            else MK_TRY(launch_bins(std::false_type{}));
+        } else if constexpr (N <= 3) {
             if (deep) MK_TRY(launch(std::true_type{}, std::false_type{}));
             else MK_TRY(launch(std::false_type{}, std::false_type{}));
         } else {

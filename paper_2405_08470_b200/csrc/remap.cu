@@ -13,7 +13,6 @@
 
 namespace mk {
 
-struct FieldMap { int src[kMaxModes]; };   // out.field[l] = in.field[src[l]]
 
 // 3-mode records are 16 B: one 128-bit load and one 128-bit store per nonzero.
 // BLOCKED: thread t handles destination position ord[t] instead of t.  `ord` lists the destination
@@ -30,9 +29,9 @@ template <bool BLOCKED>
 __global__ void __launch_bounds__(256) k_remap3(const uint4* __restrict__ in, const uint32_t* __restrict__ prev,
                                                 const uint32_t* __restrict__ ord, const uint32_t* __restrict__ osrc,
                                                 const uint8_t* __restrict__ dflags, uint4* __restrict__ out, int64_t nnz,
-                                                int64_t nnz_pad, FieldMap fm) {
+                                                int64_t nnz_pad, FieldMap fm, int64_t t0) {
     constexpr int U = remap_per_thread<BLOCKED>();
-    const int64_t base = (int64_t)blockIdx.x * (256 * U) + threadIdx.x;
+    const int64_t base = t0 + (int64_t)blockIdx.x * (256 * U) + threadIdx.x;     // t0 > 0: only the tail (padding) positions
     int64_t j[U];
     uint32_t src[U], fl[U];
     uint4 r[U];
@@ -97,18 +96,14 @@ __global__ void __launch_bounds__(256) k_remap(const uint32_t* __restrict__ in, 
 // Packed 16-byte records (common.cuh PackDesc), any N >= 4: one 128-bit load and store per nonzero.  The host
 // composes, per destination level, where its key sits in the SOURCE record (RemapPk), so the kernel unpacks
 // straight into destination order and repacks with the destination layout's offsets and flags.
-struct RemapPk {
-    int32_t soff[kMaxModes];      // bit offset of the source field in (w1:w0), or -1: it is w2 (the last key)
-    uint32_t smask[kMaxModes];
-};
 
 template <int N, bool BLOCKED>
 __global__ void __launch_bounds__(256) k_remap_pk(const uint4* __restrict__ in, const uint32_t* __restrict__ prev,
                                                   const uint32_t* __restrict__ ord, const uint32_t* __restrict__ osrc,
                                                   const uint8_t* __restrict__ dflags, uint4* __restrict__ out, int64_t nnz,
-                                                  int64_t nnz_pad, RemapPk rp, PackDesc dd) {
+                                                  int64_t nnz_pad, RemapPk rp, PackDesc dd, int64_t t0) {
     constexpr int U = remap_per_thread<BLOCKED>();
-    const int64_t base = (int64_t)blockIdx.x * (256 * U) + threadIdx.x;
+    const int64_t base = t0 + (int64_t)blockIdx.x * (256 * U) + threadIdx.x;
     int64_t j[U];
     uint32_t src[U], fl[U];
     uint4 r[U];
@@ -140,30 +135,41 @@ __global__ void __launch_bounds__(256) k_remap_pk(const uint4* __restrict__ in, 
 struct Walk { const uint32_t* map; const uint32_t* ord; const uint32_t* osrc; int blocked; };
 
 template <int N>
-static void launch_remap_n(mttkrp_handle_s* h, int from, int to, const Walk& w, unsigned grid, int64_t nnz_pad, const FieldMap& fm, cudaStream_t st) {
+static void launch_remap_n(mttkrp_handle_s* h, int from, int to, const Walk& w, unsigned grid, int64_t nnz_pad, const FieldMap& fm, cudaStream_t st,
+                           int64_t t0 = 0) {
     const ModeMeta& mf = h->mode[from];
     const uint8_t* dflags = h->mode[to].lflags;
     if constexpr (N == 3) {
-        if (w.blocked) k_remap3<true><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, w.map, w.ord, w.osrc, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, fm);
-        else k_remap3<false><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, w.map, w.ord, w.osrc, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, fm);
+        if (w.blocked) k_remap3<true><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, w.map, w.ord, w.osrc, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, fm, t0);
+        else k_remap3<false><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, w.map, w.ord, w.osrc, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, fm, t0);
     } else {
         if constexpr (N >= 4) {
             if (h->packed) {
+                FieldMap fm2;
                 RemapPk rp;
-                for (int l = 0; l < kMaxModes; ++l) { rp.soff[l] = 0; rp.smask[l] = 0; }
-                for (int l = 0; l < N; ++l) {
-                    const int sl = fm.src[l];
-                    rp.soff[l] = (sl == N - 1) ? -1 : mf.pk.off[sl];
-                    rp.smask[l] = pk_mask(mf.pk.bits[sl]);
-                }
+                remap_fields(h, from, to, &fm2, &rp);
                 const PackDesc dd = h->mode[to].pk;
-                if (w.blocked) k_remap_pk<N, true><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, w.map, w.ord, w.osrc, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, rp, dd);
-                else k_remap_pk<N, false><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, w.map, w.ord, w.osrc, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, rp, dd);
+                if (w.blocked) k_remap_pk<N, true><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, w.map, w.ord, w.osrc, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, rp, dd, t0);
+                else k_remap_pk<N, false><<<grid, 256, 0, st>>>((const uint4*)h->rec_cur, w.map, w.ord, w.osrc, dflags, (uint4*)h->rec_alt, h->nnz, nnz_pad, rp, dd, t0);
                 return;
             }
         }
         if (w.blocked) k_remap<N, true><<<grid, 256, 0, st>>>(h->rec_cur, w.map, w.ord, dflags, h->rec_alt, h->nnz, nnz_pad, fm);
         else k_remap<N, false><<<grid, 256, 0, st>>>(h->rec_cur, w.map, w.ord, dflags, h->rec_alt, h->nnz, nnz_pad, fm);
+    }
+}
+
+void remap_fields(const mttkrp_handle_s* h, int from, int to, FieldMap* fm, RemapPk* rp) {
+    const int N = h->N;
+    const ModeMeta& mf = h->mode[from];
+    for (int l = 0; l < kMaxModes; ++l) { fm->src[l] = 0; rp->soff[l] = 0; rp->smask[l] = 0; }
+    for (int l = 0; l < N; ++l) {
+        const int sl = mf.pos[h->mode[to].order[l]];
+        fm->src[l] = sl;
+        if (h->packed) {
+            rp->soff[l] = (sl == N - 1) ? -1 : mf.pk.off[sl];
+            rp->smask[l] = pk_mask(mf.pk.bits[sl]);
+        }
     }
 }
 
@@ -179,8 +185,8 @@ mttkrp_status_t launch_remap(mttkrp_handle_s* h, int from, int to, const uint32_
         if (jump) { w.map = jump; w.ord = nullptr; w.osrc = nullptr; w.blocked = 0; }
         else { w.map = mf.next; w.ord = mf.ord; w.osrc = mf.osrc; w.blocked = mf.blocked; }
         FieldMap fm;
-        for (int l = 0; l < kMaxModes; ++l) fm.src[l] = 0;
-        for (int l = 0; l < N; ++l) fm.src[l] = h->mode[from].pos[h->mode[to].order[l]];
+        RemapPk rp_unused;
+        remap_fields(h, from, to, &fm, &rp_unused);
         const int64_t nnz_pad = h->num_shards * (int64_t)h->shard_nnz;
         const int per_block = 256 * (w.blocked ? remap_per_thread<true>() : remap_per_thread<false>());
         const unsigned grid = (unsigned)((nnz_pad + per_block - 1) / per_block);
@@ -202,6 +208,32 @@ mttkrp_status_t launch_remap(mttkrp_handle_s* h, int from, int to, const uint32_
     h->rec_alt = t;
     h->cur = to;
     h->remaps_done++;
+    return MTTKRP_OK;
+}
+
+// MTTKRP_FUSE: the MTTKRP kernel scattered the nnz real records of layout `to` into rec_alt; this writes the
+// zero-valued padding records that fill the last shard (16-byte records only, plain walk from position nnz on).
+mttkrp_status_t launch_remap_padding(mttkrp_handle_s* h, int from, int to, cudaStream_t st) {
+    const int64_t nnz_pad = h->num_shards * (int64_t)h->shard_nnz;
+    if (h->nnz == 0 || nnz_pad == h->nnz) return MTTKRP_OK;
+    const ModeMeta& mf = h->mode[from];
+    Walk w;
+    w.map = mf.next; w.ord = nullptr; w.osrc = nullptr; w.blocked = 0;
+    FieldMap fm;
+    RemapPk rp_unused;
+    remap_fields(h, from, to, &fm, &rp_unused);
+    const int per_block = 256 * remap_per_thread<false>();
+    const unsigned grid = (unsigned)((nnz_pad - h->nnz + per_block - 1) / per_block);
+    switch (h->N) {
+        case 3: launch_remap_n<3>(h, from, to, w, grid, nnz_pad, fm, st, h->nnz); break;
+        case 4: launch_remap_n<4>(h, from, to, w, grid, nnz_pad, fm, st, h->nnz); break;
+        case 5: launch_remap_n<5>(h, from, to, w, grid, nnz_pad, fm, st, h->nnz); break;
+        case 6: launch_remap_n<6>(h, from, to, w, grid, nnz_pad, fm, st, h->nnz); break;
+        case 7: launch_remap_n<7>(h, from, to, w, grid, nnz_pad, fm, st, h->nnz); break;
+        case 8: launch_remap_n<8>(h, from, to, w, grid, nnz_pad, fm, st, h->nnz); break;
+        default: set_error("fused remap: unsupported nmodes %d", h->N); return MTTKRP_EUNSUPPORTED;
+    }
+    MK_CUDA(cudaGetLastError());
     return MTTKRP_OK;
 }
 

@@ -458,3 +458,36 @@ def test_out_of_order_calls_use_one_composed_pass(P):
             err, zeros_ok = oracle.normalised_error(Y, Yo, So)
             assert zeros_ok and err <= TOL
         h.destroy()
+
+
+def test_fused_remap_inside_the_compute_kernel(P, monkeypatch):
+    # SURVEY.md Sec. 8(f) f1 / Alg. 4 lines 15-19: with MTTKRP_FUSE=1 the MTTKRP kernel of mode d
+    # also executes Alg. 3 (T_out[remap id for mode (d+1) mod N] = record), so the next mode only swaps the copies.
+    # Same bars as the separate pass: the resident copy after every call is the oracle-sorted COO (bit-exact), Y
+    # within tolerance; out-of-order calls fall back to the composed gather pass.
+    monkeypatch.setenv("MTTKRP_FUSE", "1")
+    monkeypatch.setenv("MTTKRP_REMAP_BLOCK_LOG2", "12")
+    for cfg, nnz, R in [(1, 150_011, 32), (2, 120_007, 32), (3, 90_013, 16), (4, 70_001, 8), (0, 100_000, 16)]:
+        spec = W.CONFIGS[cfg].scaled(nnz)
+        t = W.generate_tensor(spec)
+        N = len(spec.dims)
+        worst, info = _run_case(P, spec.dims, t.idx, t.vals, R, seed=11, order_modes=list(range(N)) * 2 + [1, 0, N - 1, 0, 1])
+        assert info["fused_remap"] is True
+    # a full cyclic sweep costs no separate record pass: N swaps
+    spec = W.CONFIGS[1].scaled(200_003)
+    t = W.generate_tensor(spec)
+    dev = torch.device("cuda:0")
+    h = P.Mttkrp(spec.dims, t.idx.to(dev), t.vals.to(dev))
+    fac = [f.to(dev) for f in W.generate_factors(spec, 32)]
+    ref = None
+    for rep in range(3):
+        h.timing_begin()
+        outs = h.mttkrp_sweep(fac)
+        tm = h.timing_end()
+        assert tm["mttkrp_launches"] == 3
+        if ref is None:
+            ref = [y.clone() for y in outs]
+        for d in range(3):
+            assert torch.equal(outs[d], ref[d])
+    assert h.info()["remaps_done"] == 8                    # 0->1->2 in the first sweep, then 3 per sweep: all swaps
+    h.destroy()
