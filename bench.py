@@ -485,7 +485,9 @@ def run_ours(args):
     details = {"replicas": world, "checksums": case.checksums, "distinct_per_mode": case.U,
                "shard_nnz": info["shard_nnz"], "num_shards": info["num_shards"], "split_rows": info["num_split_rows"],
                "empty_rows": info["num_empty_rows"], "key_order": info["key_order"],
-               "remap_blocked": info["remap_blocked"], "remap_avg_run": [round(x, 1) for x in info["remap_avg_run"]],
+               "remap_walk": info["remap_blocked"], "remap_avg_run": [round(x, 1) for x in info["remap_avg_run"]],
+               "remap_create_time_ms": {"plain": [round(x, 3) for x in info["remap_plain_ms"]],
+                                        "two_pass": [round(x, 3) for x in info["remap_twopass_ms"]]},
                "bytes_held": info["bytes_held"], "bytes_paper_format": info["bytes_paper_format"],
                "create_s": case.create_s, "generate_s": case.generate_s}
     launches = case.launches_per_sweep * args.steps

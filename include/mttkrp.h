@@ -31,6 +31,7 @@
  *   - Process environment variables read by mttkrp_workspace_bytes / mttkrp_create (test and experiment knobs;
  *     unset = the library decides): MTTKRP_KEY_ORDER = revcyclic|desc|asc|cyclic (anything else: EINVAL),
  *     MTTKRP_PACK = 0|1, MTTKRP_REMAP_BLOCKED = 0|1, MTTKRP_REMAP_BLOCK_LOG2 (clamped to [10,26]),
+ *     MTTKRP_REMAP_TWOPASS = 0|1, MTTKRP_TWOPASS_WINDOW_LOG2 (clamped to [8,26]),
  *     MTTKRP_FORCE_DEEP = 0|1 (kernel variant), MTTKRP_FUSE = 0|1 (remap inside the MTTKRP kernel), MTTKRP_SHARD_POLICY = equal|alg1 and MTTKRP_KAPPA (number of
  *     partitions of the paper's Alg. 1 policy, default one per SM).  They must not change between the size query
  *     and create.
@@ -78,8 +79,9 @@ typedef struct {
                                          /* key_order[d] = sort-key order of the mode-d layout:
                                             key_order[d][0] == d, then the other modes (major to minor) */
     int32_t remap_blocked[MTTKRP_MAX_MODES];
-                                         /* 1: the remap d -> (d+1)%N walks the destination in source-block order
-                                            (L2-resident gather window), 0: in destination order */
+                                         /* walk of the remap d -> (d+1)%N: 0 plain (destination order), 1 blocked (destination
+                                            visited in source-block order: L2-resident gather window), 2 two passes (records
+                                            first grouped by 32 MB destination window, then gathered inside the window) */
     double remap_avg_run[MTTKRP_MAX_MODES];
                                          /* average length of the ascending destination runs of that walk */
     int32_t shard_policy;                /* 0: equal-nnz shards, rows may span blocks (default); 1: the paper's Alg. 1
@@ -87,6 +89,8 @@ typedef struct {
     int32_t kappa;                       /* partitions of the Alg. 1 policy (0 under the default policy) */
     int64_t max_partition_nnz[MTTKRP_MAX_MODES];   /* Alg. 1 policy: largest / smallest partition per mode, in nonzeros */
     int64_t min_partition_nnz[MTTKRP_MAX_MODES];
+    double remap_plain_ms[MTTKRP_MAX_MODES];       /* create-time measurement of the plain and of the two-pass walk of */
+    double remap_twopass_ms[MTTKRP_MAX_MODES];     /* that transition on this tensor (0: two passes were not a candidate) */
     int32_t fused_remap;                 /* 1: MTTKRP_FUSE=1 is in effect - the MTTKRP kernel of mode d also scatters the
                                             records into the layout of mode (d+1)%N (Alg. 4 lines 15-19) */
     int32_t reserved_;

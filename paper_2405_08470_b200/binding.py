@@ -41,6 +41,7 @@ class Info(ctypes.Structure):
                 ("remap_blocked", ctypes.c_int32 * MAX_MODES), ("remap_avg_run", ctypes.c_double * MAX_MODES),
                 ("shard_policy", ctypes.c_int32), ("kappa", ctypes.c_int32),
                 ("max_partition_nnz", ctypes.c_int64 * MAX_MODES), ("min_partition_nnz", ctypes.c_int64 * MAX_MODES),
+                ("remap_plain_ms", ctypes.c_double * MAX_MODES), ("remap_twopass_ms", ctypes.c_double * MAX_MODES),
                 ("fused_remap", ctypes.c_int32), ("reserved_", ctypes.c_int32)]
 
 
@@ -220,6 +221,7 @@ class Mttkrp:
             "key_order": [list(raw.key_order[d])[:n] for d in range(n)],
             "remap_blocked": list(raw.remap_blocked)[:n], "remap_avg_run": list(raw.remap_avg_run)[:n],
             "shard_policy": "alg1" if raw.shard_policy else "equal", "kappa": raw.kappa, "fused_remap": bool(raw.fused_remap),
+            "remap_plain_ms": list(raw.remap_plain_ms)[:n], "remap_twopass_ms": list(raw.remap_twopass_ms)[:n],
             "max_partition_nnz": list(raw.max_partition_nnz)[:n], "min_partition_nnz": list(raw.min_partition_nnz)[:n],
         }
 

@@ -380,6 +380,7 @@ mttkrp_status_t mttkrp_get_info(mttkrp_handle_t h, mttkrp_info_t* info) {
     info->bytes_held = h->bytes_held;
     info->bytes_paper_format = (h->nnz * bits + 7) / 8;
     info->remaps_done = h->remaps_done;
+    for (int m = 0; m < h->N; ++m) { info->remap_plain_ms[m] = h->mode[m].plain_ms; info->remap_twopass_ms[m] = h->mode[m].twopass_ms; }
     info->fused_remap = h->fuse;
     info->shard_policy = h->policy;
     info->kappa = h->kappa;

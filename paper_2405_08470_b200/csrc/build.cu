@@ -358,6 +358,12 @@ __global__ void k_gather_u8(const uint8_t* __restrict__ table, const uint32_t* _
     if (k < n) out[k] = table[idx[k]];
 }
 
+// out[b[a[m]]] = m
+__global__ void k_invert_through(const uint32_t* __restrict__ a, const uint32_t* __restrict__ b, uint32_t* __restrict__ out, int64_t n) {
+    int64_t m = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m < n) out[b[a[m]]] = (uint32_t)m;
+}
+
 // key[j] = map[j] >> shift (the source block of destination position j)
 __global__ void k_block_keys(const uint32_t* __restrict__ map, int shift, uint32_t* __restrict__ key, int64_t n) {
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -754,6 +760,65 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
         if (benv) blocked = nnz > 0 && benv[0] == '1';
         h->mode[d].blocked = blocked ? 1 : 0;
         h->mode[d].avg_run = nnz > 0 ? (double)nnz / (double)runs : 0.0;
+        h->mode[d].plain_ms = h->mode[d].twopass_ms = 0.f;
+    }
+    // Two-pass remap for the transitions that stay a random gather (16-byte records, tensors of many windows): build
+    // the two maps into the (otherwise unused) ord / osrc arrays, then TIME one cycle of transitions with the plain
+    // walk and one with the two passes on the real tensor and keep, per transition, the faster one.
+    const char* tenv = getenv("MTTKRP_REMAP_TWOPASS");          // 0 / 1 force the choice (tests, experiments)
+    const bool tp_forced_on = tenv && tenv[0] == '1', tp_forced_off = (tenv && tenv[0] == '0') || benv;
+    bool cand[kMaxModes] = {false};
+    bool any_cand = false;
+    if (nnz > 0 && h->rec_words == 4 && !tp_forced_off) {
+        int wlog = kTwoPassWindowLog2;
+        if (const char* wenv = getenv("MTTKRP_TWOPASS_WINDOW_LOG2")) wlog = std::min(26, std::max(8, atoi(wenv)));   // tests
+        while ((nnz >> wlog) > 255) ++wlog;
+        for (int d = 0; d < N; ++d) {
+            const int64_t src_runs = (int64_t)breaks[kMaxModes + d] + 1;
+            const bool random_gather = (double)nnz / (double)src_runs < 1.5;
+            cand[d] = !h->mode[d].blocked && (tp_forced_on || (random_gather && (nnz >> wlog) >= 8));
+            if (!cand[d]) continue;
+            any_cand = true;
+            ModeMeta& mm = h->mode[d];
+            mm.block_log2 = wlog;                                     // two-pass walk: log2 of the destination window
+            uint32_t* scat = permB;                                   // inverse of next: destination of source position s
+            k_invert<<<grid_for(nnz, 256), 256, 0, st>>>(mm.next, scat, nnz);
+            k_block_keys<<<grid_for(nnz, 256), 256, 0, st>>>(scat, wlog, keyA, nnz);
+            k_iota<<<grid_for(nnz, 256), 256, 0, st>>>(permA, nnz);
+            k_radix_hist<<<(unsigned)nblocks, kSortThreads, 0, st>>>(keyA, nnz, 0, hist, nblocks);
+            MK_TRY(exclusive_scan(hist, 256 * nblocks, sums, st));
+            // mm.osrc = source positions grouped (stably) by destination window = the order of the intermediate copy
+            k_radix_scatter<<<(unsigned)nblocks, kSortThreads, 0, st>>>(keyA, permA, keyB, mm.osrc, nnz, 0, hist, nblocks);
+            k_invert<<<grid_for(nnz, 256), 256, 0, st>>>(mm.osrc, mm.ord, nnz);                    // s1[s] = slot of source s
+            k_invert_through<<<grid_for(nnz, 256), 256, 0, st>>>(mm.osrc, scat, keyA, nnz);        // g2[t] = slot of destination t
+            MK_CUDA(cudaMemcpyAsync(mm.osrc, keyA, 4 * n, cudaMemcpyDeviceToDevice, st));
+        }
+        MK_CUDA(cudaGetLastError());
+    }
+    if (any_cand) {
+        cudaEvent_t e0, e1;
+        MK_CUDA(cudaEventCreate(&e0));
+        MK_CUDA(cudaEventCreate(&e1));
+        for (int pass = 0; pass < 3; ++pass) {                  // warm-up cycle, plain cycle, two-pass cycle
+            for (int d = 0; d < N; ++d) {
+                h->mode[d].blocked = (pass == 2 && cand[d]) ? 2 : (h->mode[d].blocked == 1 ? 1 : 0);
+                MK_CUDA(cudaEventRecord(e0, st));
+                MK_TRY(launch_remap(h, d, (d + 1) % N, nullptr, st));
+                MK_CUDA(cudaEventRecord(e1, st));
+                MK_CUDA(cudaEventSynchronize(e1));
+                float ms = 0.f;
+                MK_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+                if (pass == 1) h->mode[d].plain_ms = cand[d] ? ms : 0.f;
+                if (pass == 2) h->mode[d].twopass_ms = cand[d] ? ms : 0.f;
+            }
+        }
+        cudaEventDestroy(e0);
+        cudaEventDestroy(e1);
+        for (int d = 0; d < N; ++d) {
+            if (!cand[d]) continue;
+            h->mode[d].blocked = (tp_forced_on || h->mode[d].twopass_ms < 0.95f * h->mode[d].plain_ms) ? 2 : 0;
+        }
+        h->remaps_done = 0;                                      // the tensor is back in the mode-0 layout (N transitions per cycle)
     }
     return MTTKRP_OK;
 }

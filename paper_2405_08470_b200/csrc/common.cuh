@@ -102,7 +102,9 @@ struct ModeMeta {
                               // in this order so that its random reads stay inside one L2-resident window at a time
     uint32_t* osrc;           // [nnz] osrc[t] = next[ord[t]]: the source position of walk step t (saves the walk one
                               // dependent gather)
-    int blocked;              // 1: the remap d -> (d+1)%N uses `ord`
+    int blocked;              // walk of the remap d -> (d+1)%N: 0 plain (destination order), 1 blocked (`ord`/`osrc`), 2 two
+                              // passes (ord = scatter map into the window-grouped intermediate copy, osrc = gather map out of it)
+    float plain_ms, twopass_ms;   // create-time measurements behind the choice of 2 (0 when not a candidate)
     int block_log2;
     double avg_run;           // average length of the ascending destination runs in `ord`
     uint8_t* lflags;          // [nnz_pad] run-end flags of THIS layout: bit l = e_l (see "Run-end flags")
@@ -216,6 +218,7 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
 
 // ---- remap.cu -------------------------------------------------------------------------------
 mttkrp_status_t launch_remap(mttkrp_handle_s* h, int from, int to, const uint32_t* jump, cudaStream_t st);   // swaps copies
+constexpr int kTwoPassWindowLog2 = 21;      // destination window of the two-pass remap: 2^21 records (32 MB), L2-resident
 void remap_fields(const mttkrp_handle_s* h, int from, int to, FieldMap* fm, RemapPk* rp);
 mttkrp_status_t launch_remap_padding(mttkrp_handle_s* h, int from, int to, cudaStream_t st);   // padding records of rec_alt only
 mttkrp_status_t launch_export(const mttkrp_handle_s* h, int32_t* idx, float* vals, cudaStream_t st);

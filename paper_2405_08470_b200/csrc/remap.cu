@@ -159,6 +159,71 @@ static void launch_remap_n(mttkrp_handle_s* h, int from, int to, const Walk& w, 
     }
 }
 
+// Pass 1 of the two-pass remap (16-byte records): mid[s1[s]] = in[s].  The intermediate copy groups the records by
+// the 2^21-record window of the destination layout they go to, in source order inside a window: the source is read
+// once, sequentially, and every block appends a contiguous run to each of the ~100 window streams, which L2 merges
+// into whole lines.  Pass 2 is the plain gather walk out of `mid`: its random reads stay inside one window (32 MB).
+// A block takes a tile of kScatterTile consecutive source records.  Inside a window the intermediate order is the
+// source order, so the tile's records for one window occupy CONSECUTIVE slots of `mid`: the block sorts its tile by
+// window in shared memory (histogram + first slot per window) and then writes it out in that order, consecutive lanes
+// to consecutive addresses, i.e. whole sectors and lines instead of 16-byte pieces.
+constexpr int kScatterTile = 2048;
+__global__ void __launch_bounds__(256) k_scatter16(const uint4* __restrict__ in, const uint32_t* __restrict__ s1,
+                                                   uint4* __restrict__ mid, int64_t nnz, int wlog) {
+    __shared__ uint4 s_rec[kScatterTile];
+    __shared__ uint32_t s_dst[kScatterTile];
+    __shared__ uint32_t s_cnt[256], s_first[256], s_off[256];
+    const int64_t base = (int64_t)blockIdx.x * kScatterTile;
+    const int n = (int)min((int64_t)kScatterTile, nnz - base);
+    s_cnt[threadIdx.x] = 0;
+    s_first[threadIdx.x] = 0xffffffffu;
+    __syncthreads();
+    constexpr int PER = kScatterTile / 256;
+    uint4 r[PER];
+    uint32_t dst[PER];
+#pragma unroll
+    for (int i = 0; i < PER; ++i) {
+        const int j = threadIdx.x + i * 256;
+        if (j < n) {
+            dst[i] = __ldcs(s1 + base + j);
+            r[i] = __ldcs(in + base + j);
+            const uint32_t w = dst[i] >> wlog;
+            atomicAdd(&s_cnt[w], 1u);
+            atomicMin(&s_first[w], dst[i]);
+        }
+    }
+    __syncthreads();
+    {   // exclusive scan of the 256 window counts (one warp, 8 per lane)
+        if (threadIdx.x < 32) {
+            uint32_t v[8], sum = 0;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) { v[q] = s_cnt[threadIdx.x * 8 + q]; sum += v[q]; }
+            uint32_t inc = sum;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+                if ((int)threadIdx.x >= o) inc += t;
+            }
+            uint32_t run = inc - sum;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) { s_off[threadIdx.x * 8 + q] = run; run += v[q]; }
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < PER; ++i) {
+        const int j = threadIdx.x + i * 256;
+        if (j < n) {
+            const uint32_t w = dst[i] >> wlog;
+            const uint32_t slot = s_off[w] + (dst[i] - s_first[w]);
+            s_rec[slot] = r[i];
+            s_dst[slot] = dst[i];
+        }
+    }
+    __syncthreads();
+    for (int j = threadIdx.x; j < n; j += 256) mid[s_dst[j]] = s_rec[j];
+}
+
 void remap_fields(const mttkrp_handle_s* h, int from, int to, FieldMap* fm, RemapPk* rp) {
     const int N = h->N;
     const ModeMeta& mf = h->mode[from];
@@ -183,6 +248,14 @@ mttkrp_status_t launch_remap(mttkrp_handle_s* h, int from, int to, const uint32_
         const ModeMeta& mf = h->mode[from];
         Walk w;
         if (jump) { w.map = jump; w.ord = nullptr; w.osrc = nullptr; w.blocked = 0; }
+        else if (mf.blocked == 2) {
+            // two passes: group by destination window into the other copy, then gather out of it into this one
+            TimedLaunch tl(h->timing, kClsRemap, st);
+            k_scatter16<<<(unsigned)((h->nnz + kScatterTile - 1) / kScatterTile), 256, 0, st>>>((const uint4*)h->rec_cur, mf.ord, (uint4*)h->rec_alt, h->nnz,
+                                                                                           mf.block_log2);
+            uint32_t* t = h->rec_cur; h->rec_cur = h->rec_alt; h->rec_alt = t;
+            w.map = mf.osrc; w.ord = nullptr; w.osrc = nullptr; w.blocked = 0;
+        }
         else { w.map = mf.next; w.ord = mf.ord; w.osrc = mf.osrc; w.blocked = mf.blocked; }
         FieldMap fm;
         RemapPk rp_unused;

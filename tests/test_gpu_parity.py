@@ -248,6 +248,22 @@ def test_remap_walks_and_key_orders(P, monkeypatch, order, blocked):
             assert info["key_order"] == [[(d - j) % N for j in range(N)] for d in range(N)]
 
 
+@pytest.mark.parametrize("order", ["revcyclic", "desc"])
+def test_two_pass_remap(P, monkeypatch, order):
+    # The third walk of Alg. 3: records first grouped by destination window (scatter, sequential reads), then gathered
+    # inside the window.  Same contract as the other walks: permutation, remapped copy and Y equal the oracle's.
+    monkeypatch.setenv("MTTKRP_KEY_ORDER", order)
+    monkeypatch.setenv("MTTKRP_REMAP_TWOPASS", "1")
+    monkeypatch.setenv("MTTKRP_TWOPASS_WINDOW_LOG2", "11")          # many windows even at test sizes
+    for cfg, nnz, R in [(1, 150_001, 32), (2, 260_003, 32), (3, 90_007, 16), (4, 60_013, 8)]:
+        spec = W.CONFIGS[cfg].scaled(nnz)
+        t = W.generate_tensor(spec)
+        N = len(spec.dims)
+        worst, info = _run_case(P, spec.dims, t.idx, t.vals, R, seed=6, order_modes=list(range(N)) + [0, N - 1, 1, 2, 0])
+        assert 2 in info["remap_blocked"] and info["remaps_done"] == 0
+        assert all(w == 2 or w == 1 for w in info["remap_blocked"])
+
+
 @pytest.mark.parametrize("pack", ["0", "1"])
 def test_record_formats_for_four_and_more_modes(P, monkeypatch, pack):
     # N >= 4: packed 16-byte records (bit-level layout) and the 4*(N+1)-byte fallback
