@@ -87,9 +87,35 @@ __device__ __forceinline__ uint64_t l2_policy_evict_first() {
 // One lane's 4 columns of a factor row (read-only path, 128-bit load).  `base` = this lane's slot in row 0 of
 // the factor matrix (float4 units), `key` = row index, LPN = lanes per row: the address is one 32x32->64
 // multiply-add on a per-lane base.  Needs dims[m] < 2^28 (api.cu check_shape).
+#ifndef MK_ROWPOL        // experiment: L2 eviction policy of the factor-row gathers. 0 = default; 1 = evict_last with fraction
+#define MK_ROWPOL 0      // MK_ROWPOL_FRAC on all rows; 2 = on fiber-level rows only; 3 = evict_first on last-level rows only
+#endif
+#ifndef MK_ROWPOL_FRAC
+#define MK_ROWPOL_FRAC 0.5
+#endif
+#define MK_STR2(x) #x
+#define MK_STR(x) MK_STR2(x)
+__device__ __forceinline__ float4 ldg_pol(const float4* p, int kind) {   // kind 0: last level, 1: fiber level
+#if MK_ROWPOL == 0
+    (void)kind;
+    return __ldg(p);
+#else
+    float4 v;
+    const bool last_pol = (MK_ROWPOL == 1 || MK_ROWPOL == 3), fiber_pol = (MK_ROWPOL == 1 || MK_ROWPOL == 2);
+    if ((kind == 0 && last_pol) || (kind == 1 && fiber_pol)) {
+        uint64_t pol;
+        if (MK_ROWPOL == 3) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+        else asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, " MK_STR(MK_ROWPOL_FRAC) ";" : "=l"(pol));
+        asm volatile("ld.global.nc.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p), "l"(pol));
+    } else {
+        v = __ldg(p);
+    }
+    return v;
+#endif
+}
 template <int LPN>
 __device__ __forceinline__ Vec ld_row(const float4* __restrict__ base, uint32_t key) {
-    const float4 v = __ldg(base + (size_t)key * LPN);
+    const float4 v = ldg_pol(base + (size_t)key * LPN, 0);
     Vec r;
     r.p[0] = make_float2(v.x, v.y);
     r.p[1] = make_float2(v.z, v.w);
@@ -102,7 +128,7 @@ template <int LPN>
 __device__ __forceinline__ Vec ld_row_flagged(const float* __restrict__ base, uint32_t word, uint32_t sub) {
     constexpr int SH = LPN == 16 ? 4 : (LPN == 8 ? 3 : (LPN == 4 ? 2 : 1));
     const uint32_t off = (word << SH) + sub;
-    const float4 v = __ldg(reinterpret_cast<const float4*>(base) + off);
+    const float4 v = ldg_pol(reinterpret_cast<const float4*>(base) + off, 1);
     Vec r;
     r.p[0] = make_float2(v.x, v.y);
     r.p[1] = make_float2(v.z, v.w);
