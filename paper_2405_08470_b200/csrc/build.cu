@@ -27,6 +27,7 @@ constexpr int kSortTile = kSortThreads * kSortItems;   // keys per block per rad
 constexpr int kScanThreads = 256;
 constexpr int kScanItems = 8;
 constexpr int kScanTile = kScanThreads * kScanItems;
+constexpr int kDegBins = 1024;                          // bins of the degree histogram behind the cold-row marks (deg_bin)
 
 int device_sm_count() {
     int dev = 0, sms = 0;
@@ -85,6 +86,8 @@ mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_
     scratch += 2 * align_up(4 * ((size_t)std::max<int64_t>(maxdim, p->num_shards) + 1));   // flags + positions
     scratch += align_up(4 * (std::max<size_t>(256 * nblocks + 1, (size_t)maxdim + 1) / kScanTile + 2));  // scan block sums
     scratch += 4096;                                                  // counters, error flag
+    for (int d = 0; d < N; ++d) scratch += align_up(4 * ((size_t)dims[d] + 1));   // index degrees (cold-row marks)
+    scratch += align_up(4 * kDegBins);                                // degree histogram
     p->total = off + std::max(align_up(rec_bytes), scratch);
     return MTTKRP_OK;
 }
@@ -106,6 +109,40 @@ __global__ void k_validate(const int32_t* __restrict__ idx, int64_t nnz, int N, 
 __global__ void k_count_keys(const uint32_t* __restrict__ key, int64_t n, uint32_t* __restrict__ deg) {
     int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k < n) atomicAdd(deg + key[k], 1u);
+}
+
+// Same count with the lanes of a warp that hit the same key combined first (Zipf-skewed modes put a fifth of the
+// nonzeros on one counter).
+__global__ void k_count_keys_agg(const uint32_t* __restrict__ key, int64_t n, uint32_t* __restrict__ deg) {
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool in = k < n;
+    const uint32_t v = in ? key[k] : 0xffffffffu;
+    const unsigned peers = __match_any_sync(0xffffffffu, v);
+    if (in && (int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(deg + v, (uint32_t)__popc(peers));
+}
+
+// Degree histogram on a log-linear scale (exact below 64, then 32 steps per octave): the host reads it to turn
+// "the K most frequent rows" into a degree threshold (cold-row marks, common.cuh).
+__host__ __device__ inline int deg_bin(uint32_t deg) {
+    if (deg < 64u) return (int)deg;
+    int lg = 31;
+    while (!((deg >> lg) & 1u)) --lg;                   // floor(log2 deg) >= 6
+    return 64 + (lg - 6) * 32 + (int)((deg >> (lg - 5)) & 31u);
+}
+__host__ __device__ inline uint32_t deg_bin_floor(int bin) {      // smallest degree that falls into `bin`
+    if (bin < 64) return (uint32_t)bin;
+    const int lg = (bin - 64) / 32 + 6, sub = (bin - 64) % 32;
+    return (uint32_t)(32 + sub) << (lg - 5);
+}
+__global__ void k_degree_hist(const uint32_t* __restrict__ deg, int64_t rows, uint32_t* __restrict__ hist) {
+    __shared__ uint32_t h[kDegBins];
+    for (int i = threadIdx.x; i < kDegBins; i += blockDim.x) h[i] = 0;
+    __syncthreads();
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < rows; i += (int64_t)gridDim.x * blockDim.x)
+        atomicAdd(&h[deg_bin(deg[i])], 1u);
+    __syncthreads();
+    for (int i = threadIdx.x; i < kDegBins; i += blockDim.x)
+        if (h[i]) atomicAdd(hist + i, h[i]);
 }
 
 __global__ void k_iota(uint32_t* __restrict__ p, int64_t n) {
@@ -302,8 +339,14 @@ struct OrderArg { int v[kMaxModes]; };
 // Run-end flags of one layout (common.cuh): bit l of flags[k] = e_l = "the record at k+1 differs from
 // the record at k in one of the keys k_0..k_l".  Padding positions repeat the last nonzero (no run
 // ends); the last position of the padded array has every flag set.
+// For N <= 3 the byte also carries the cold-row marks (common.cuh): bit 6 = the last-level row, bit 7 = the fiber-level
+// row (N = 3) is cold, i.e. its index occurs fewer than cold.t[c] times in the tensor.  cold.deg[c] == nullptr: no marks.
+struct ColdArg {
+    const uint32_t* deg[2];
+    uint32_t t[2];
+};
 __global__ void k_build_flags(const int32_t* __restrict__ idx, const uint32_t* __restrict__ perm, int64_t nnz,
-                              int64_t nnz_pad, int N, OrderArg order, uint8_t* __restrict__ flags) {
+                              int64_t nnz_pad, int N, OrderArg order, ColdArg cold, uint8_t* __restrict__ flags) {
     int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= nnz_pad) return;
     const bool last = k + 1 >= nnz_pad;
@@ -315,6 +358,13 @@ __global__ void k_build_flags(const int32_t* __restrict__ idx, const uint32_t* _
         const size_t col = (size_t)order.v[l] * nnz;
         diff = diff || (idx[col + src] != idx[col + nsrc]);
         f |= (diff ? 1u : 0u) << l;
+    }
+    if (N <= 3) {
+        for (int c = 0; c < N - 1; ++c) {                // c = 0: last level (key N-1), c = 1: fiber level (key N-2)
+            if (!cold.deg[c]) continue;
+            const uint32_t dg = cold.deg[c][idx[(size_t)order.v[N - 1 - c] * nnz + src]];
+            f |= (dg < cold.t[c] ? 1u : 0u) << (6 + c);
+        }
     }
     flags[k] = (uint8_t)f;
 }
@@ -333,6 +383,8 @@ __global__ void k_build_records(const int32_t* __restrict__ idx, const float* __
     for (int l = 0; l < N; ++l) {
         uint32_t key = (uint32_t)idx[(size_t)order.v[l] * nnz + src];
         if (l <= N - 2) key |= ((f >> l) & 1u) << 31;                  // e_l rides on key word l (common.cuh)
+        if (N <= 3 && l == 0) key |= ((f >> 6) & 1u) << 30;             // cold-row mark of the last-level row
+        if (N == 3 && l == 1) key |= ((f >> 7) & 1u) << 30;             // ... of the fiber-level row
         r[l] = key;
     }
     r[N] = k < nnz ? __float_as_uint(vals[src]) : 0u;
@@ -564,6 +616,9 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
     uint32_t* sums = (uint32_t*)take(4 * (std::max<size_t>(256 * (size_t)nblocks + 1, (size_t)maxdim + 1) / kScanTile + 2));
     uint32_t* small = (uint32_t*)take(4096);          // [0]=bad flag, [8..8+2N) counts, then dims
     int64_t* dims_dev = (int64_t*)(small + 64);
+    uint32_t* degs[kMaxModes];
+    for (int d = 0; d < N; ++d) degs[d] = (uint32_t*)take(4 * ((size_t)h->dims[d] + 1));
+    uint32_t* dhist = (uint32_t*)take(4 * kDegBins);
 
     MK_CUDA(cudaMemsetAsync(small, 0, 4096, st));
     MK_CUDA(cudaMemcpyAsync(dims_dev, h->dims, sizeof(int64_t) * N, cudaMemcpyHostToDevice, st));
@@ -578,6 +633,32 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
         if (bad) {
             set_error("index out of range in mode mask 0x%x", bad);
             return MTTKRP_EINDEX;
+        }
+    }
+
+    // Cold-row marks (common.cuh; unpacked records, N <= 3): degree of every index of every mode, and per mode the
+    // degree below which a row is not among the K = MTTKRP_PREFETCH_ROWS most frequent ones (0 switches the marks off).
+    for (int m = 0; m < N; ++m) { h->cold_deg[m] = 0; h->cold_rows[m] = 0; }
+    int64_t k_keep = 65536;
+    if (const char* e = getenv("MTTKRP_PREFETCH_ROWS")) k_keep = std::max<long long>(0, atoll(e));
+    const bool marks = nnz > 0 && N <= 3 && !h->packed && k_keep > 0;
+    if (marks) {
+        uint32_t hh[kDegBins];
+        for (int m = 0; m < N; ++m) {
+            const int64_t rows = h->dims[m];
+            if (rows <= k_keep) continue;                        // every row is kept
+            MK_CUDA(cudaMemsetAsync(degs[m], 0, 4 * (size_t)(rows + 1), st));
+            MK_CUDA(cudaMemsetAsync(dhist, 0, 4 * kDegBins, st));
+            k_count_keys_agg<<<grid_for(nnz, 256), 256, 0, st>>>((const uint32_t*)idx + (size_t)m * n, nnz, degs[m]);
+            k_degree_hist<<<(unsigned)std::min<int64_t>(grid_for(rows, 256), 1024), 256, 0, st>>>(degs[m], rows, dhist);
+            MK_CUDA(cudaMemcpyAsync(hh, dhist, 4 * kDegBins, cudaMemcpyDeviceToHost, st));
+            MK_CUDA(cudaStreamSynchronize(st));
+            // smallest bin boundary T with #{rows of degree >= T} <= K: rows of degree < T are cold
+            int64_t cum = 0;
+            int b = kDegBins;
+            while (b > 0 && cum + hh[b - 1] <= k_keep) { cum += hh[b - 1]; --b; }
+            h->cold_deg[m] = b >= kDegBins ? 0xffffffffu : deg_bin_floor(b);
+            h->cold_rows[m] = rows - cum;
         }
     }
 
@@ -646,7 +727,15 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
                 OrderArg oa;
                 for (int l = 0; l < kMaxModes; ++l) oa.v[l] = mm.order[l];
                 const int64_t nnz_pad = nshards * (int64_t)S;
-                k_build_flags<<<grid_for(nnz_pad, 256), 256, 0, st>>>(idx, pa, nnz, nnz_pad, N, oa, mm.lflags);
+                ColdArg ca;
+                ca.deg[0] = ca.deg[1] = nullptr;
+                ca.t[0] = ca.t[1] = 0;
+                if (marks) {
+                    const int ml = mm.order[N - 1];
+                    if (h->cold_deg[ml]) { ca.deg[0] = degs[ml]; ca.t[0] = h->cold_deg[ml]; }
+                    if (N == 3) { const int mf = mm.order[1]; if (h->cold_deg[mf]) { ca.deg[1] = degs[mf]; ca.t[1] = h->cold_deg[mf]; } }
+                }
+                k_build_flags<<<grid_for(nnz_pad, 256), 256, 0, st>>>(idx, pa, nnz, nnz_pad, N, oa, ca, mm.lflags);
             }
             MK_CUDA(cudaMemcpyAsync(dst, pa, 4 * n, cudaMemcpyDeviceToDevice, st));
             if (d == 0) MK_CUDA(cudaMemcpyAsync(h->perm0, pa, 4 * n, cudaMemcpyDeviceToDevice, st));

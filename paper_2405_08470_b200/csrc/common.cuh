@@ -39,14 +39,29 @@ void set_error(const char* fmt, ...);
 // loop turns it into an address with one multiply-add.  Padding records repeat the keys of the last
 // nonzero (no run ends); the very last record of the padded array has every flag set.
 constexpr uint32_t kFlag = 0x80000000u;
-constexpr uint32_t kKeyMask = 0x7fffffffu;
+constexpr uint32_t kKeyMask = 0x0fffffffu;           // indices are < 2^28 (api.cu check_shape): bits 28..31 of a key word are free
 
-// The flags are a property of (layout, position), so mttkrp_create computes them once per layout into a
-// byte array (bit l = e_l) and the record builder / remap pass only merges them into the key words.
+// Cold-row marks (unpacked records, N <= 3).  The tensor is fixed, so which factor rows are re-used often is known
+// before the first MTTKRP: mttkrp_create counts how often every index of a mode occurs (its degree) and calls a row
+// COLD when it is not among the K most frequent rows of its factor matrix (K = MTTKRP_PREFETCH_ROWS, default 65536
+// rows = 8 MB at R = 32; a factor with fewer rows has no cold row).  A gather of a cold row almost always misses L2
+// when the factor matrices overflow it, and that miss decides how long the whole batch of gathers waits.  The
+// record carries the mark for the row it gathers at the last level in bit 30 of key word 0 (word 0 is in a register
+// in the hot loop anyway; the last key word itself stays flag-free) and, N = 3, for the row of its fiber level in
+// bit 30 of key word 1.  The MTTKRP kernel requests marked rows into L2 one ring stage ahead (mttkrp_kernel.cu).
+constexpr uint32_t kCold = 1u << 30;
+
+// The flags are a property of (layout, position), so mttkrp_create computes them once per layout into a byte array
+// and the record builder / remap pass only merges them into the key words.  Byte layout: bit l = e_l (l <= N-2); for
+// N <= 3 also bit 6 = last-level row cold, bit 7 = fiber-level row cold.
 template <int N>
 __device__ __forceinline__ void apply_run_flags(uint32_t* k, uint32_t f) {
 #pragma unroll
     for (int l = 0; l < N - 1; ++l) k[l] |= ((f >> l) & 1u) << 31;
+    if constexpr (N <= 3) {
+        k[0] |= ((f >> 6) & 1u) << 30;
+        if constexpr (N == 3) k[1] |= ((f >> 7) & 1u) << 30;
+    }
 }
 
 // Packed 16-byte records (N >= 4).  When the index widths allow, a record is {w0, w1, w2, val}: the keys of
@@ -174,6 +189,8 @@ struct mttkrp_handle_s {
     int device;
     int num_sms;              // SM count of `device` (grid sizing)
     int force_deep;           // MTTKRP_FORCE_DEEP at create: -1 = by factor size (default), 0 / 1 = never / always
+    uint32_t cold_deg[mk::kMaxModes];   // cold-row marks: a row of mode m is cold when its index occurs fewer than this many times (0: none)
+    int64_t cold_rows[mk::kMaxModes];   // ... and how many rows of the mode that makes
     cudaStream_t last_stream; // stream of the last call that launched work for this handle
     cudaEvent_t ev_order;     // recorded on last_stream after every such call: a call on another stream waits on it
     int launched;             // ev_order has been recorded at least once
