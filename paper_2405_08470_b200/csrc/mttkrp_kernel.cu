@@ -127,7 +127,7 @@ __device__ __forceinline__ Vec ld_row(const float4* __restrict__ base, uint32_t 
 template <int LPN>
 __device__ __forceinline__ Vec ld_row_flagged(const float* __restrict__ base, uint32_t word, uint32_t sub) {
     constexpr int SH = LPN == 16 ? 4 : (LPN == 8 ? 3 : (LPN == 4 ? 2 : 1));
-    const uint32_t off = (word << SH) + sub;
+    const uint32_t off = ((SH >= 2 ? word : (word & kKeyMask)) << SH) + sub;      // the shift drops bits 30 / 31 (flag, cold mark)
     const float4 v = ldg_pol(reinterpret_cast<const float4*>(base) + off, 1);
     Vec r;
     r.p[0] = make_float2(v.x, v.y);
@@ -169,6 +169,16 @@ __device__ __forceinline__ uint4 lds128(uint32_t addr) {
     uint4 v;
     asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
     return v;
+}
+// Requests the line of a factor row into L2 (SASS CCTL.E.PF2: no register, no scoreboard).
+#ifndef MK_PREFETCH      // 0: off; 1: one request per row; 2: both 64-byte halves
+#define MK_PREFETCH 1
+#endif
+__device__ __forceinline__ void prefetch_l2(const float4* row) {
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(row));
+#if MK_PREFETCH >= 2
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(row + 4));
+#endif
 }
 __device__ __forceinline__ uint32_t lds32(uint32_t addr) {
     uint32_t v;
@@ -380,7 +390,11 @@ __device__ __forceinline__ void shard_body(const KernelArgs<N>& a, const int64_t
             // steps are read with back-to-back LDS.128, their B last-level rows and up to B fiber rows are requested
             // together (up to 8 independent 128-bit gathers per lane in flight), then the B steps are computed.  Costs
             // 64 registers (4 blocks per SM); one vote per batch replaces the per-step output-row-end test.
-            constexpr int B = 4;
+#ifndef MK_B
+#define MK_B 4
+#endif
+            constexpr int B = MK_B;
+            static_assert(K % B == 0, "batch");
             Vec al[B], rb[B];
             float val[B];
             bool e1[B];
@@ -439,10 +453,33 @@ __device__ __forceinline__ void shard_body(const KernelArgs<N>& a, const int64_t
                 const int nstage = (stage + 1 == STAGES) ? 0 : stage + 1;
                 const uint32_t cs = ring_gs + 4u * (uint32_t)(stage * STAGEW);
                 const uint32_t ns = ring_gs + 4u * (uint32_t)(nstage * STAGEW);
-                C(cs);
-                P(cs + 4u * (uint32_t)(B * ROWW));
-                C(cs + 4u * (uint32_t)(B * ROWW));
-                if (r + 1 < nrounds) P(ns);
+#if MK_PREFETCH
+                // Cold rows (common.cuh: outside the K most frequent of their factor matrix, so they almost always miss
+                // L2 when the factors overflow it) of the NEXT round are requested into L2 now, one round (~3000 clk)
+                // before their gathers; lane p of the group looks at record p of that round.  The batch then waits for
+                // L2 hits instead of HBM reads (configs[2]: -7 % per mode).
+                if (r + 1 < nrounds) {
+#pragma unroll
+                    for (int i = 0; i < (K + LPN - 1) / LPN; ++i) {
+                        const int pr = sub + i * LPN;
+                        if (K % LPN == 0 || pr < K) {
+                            const uint4 q = lds128(ns + 4u * (uint32_t)(pr * ROWW));
+                            const uint32_t klast = N == 3 ? q.z : q.y;
+                            if (q.x & kCold) prefetch_l2(reinterpret_cast<const float4*>(a.fac[N - 1]) + (size_t)klast * LPN);
+                            if constexpr (N == 3) {
+                                if ((int32_t)q.y < 0 && (q.y & kCold))
+                                    prefetch_l2(reinterpret_cast<const float4*>(a.fac[1]) + (size_t)(q.y & kKeyMask) * LPN);
+                            }
+                        }
+                    }
+                }
+#endif
+#pragma unroll
+                for (int b = 0; b < K / B; ++b) {
+                    C(cs + 4u * (uint32_t)(b * B * ROWW));
+                    if (b + 1 < K / B) P(cs + 4u * (uint32_t)((b + 1) * B * ROWW));
+                    else if (r + 1 < nrounds) P(ns);
+                }
                 stage = nstage;
                 __syncwarp();                                 // everyone is done with round r's stage
             }
