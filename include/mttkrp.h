@@ -32,7 +32,8 @@
  *     unset = the library decides): MTTKRP_KEY_ORDER = revcyclic|desc|asc|cyclic (anything else: EINVAL),
  *     MTTKRP_PACK = 0|1, MTTKRP_REMAP_BLOCKED = 0|1, MTTKRP_REMAP_BLOCK_LOG2 (clamped to [10,26]),
  *     MTTKRP_REMAP_TWOPASS = 0|1, MTTKRP_TWOPASS_WINDOW_LOG2 (clamped to [8,26]),
- *     MTTKRP_FORCE_DEEP = 0|1 (kernel variant), MTTKRP_FUSE = 0|1 (remap inside the MTTKRP kernel), MTTKRP_SHARD_POLICY = equal|alg1 and MTTKRP_KAPPA (number of
+ *     MTTKRP_FORCE_DEEP = 0|1 (kernel variant), MTTKRP_PREFETCH_ROWS (rows per factor matrix that are NOT prefetched
+ *     into L2, default 65536; 0 = no prefetch), MTTKRP_FUSE = 0|1 (remap inside the MTTKRP kernel), MTTKRP_SHARD_POLICY = equal|alg1 and MTTKRP_KAPPA (number of
  *     partitions of the paper's Alg. 1 policy, default one per SM).  They must not change between the size query
  *     and create.
  */
@@ -94,6 +95,10 @@ typedef struct {
     int32_t fused_remap;                 /* 1: MTTKRP_FUSE=1 is in effect - the MTTKRP kernel of mode d also scatters the
                                             records into the layout of mode (d+1)%N (Alg. 4 lines 15-19) */
     int32_t reserved_;
+    int64_t cold_rows[MTTKRP_MAX_MODES]; /* cold-row marks (nmodes <= 3): rows of mode m that are NOT among the
+                                            MTTKRP_PREFETCH_ROWS most frequent ones (0: the factor has no cold row); the
+                                            MTTKRP kernel requests such rows into L2 ahead of their gathers */
+    int64_t cold_degree[MTTKRP_MAX_MODES];/* ... a row of mode m is cold when its index occurs fewer than this many times */
 } mttkrp_info_t;
 
 /*

@@ -42,7 +42,8 @@ class Info(ctypes.Structure):
                 ("shard_policy", ctypes.c_int32), ("kappa", ctypes.c_int32),
                 ("max_partition_nnz", ctypes.c_int64 * MAX_MODES), ("min_partition_nnz", ctypes.c_int64 * MAX_MODES),
                 ("remap_plain_ms", ctypes.c_double * MAX_MODES), ("remap_twopass_ms", ctypes.c_double * MAX_MODES),
-                ("fused_remap", ctypes.c_int32), ("reserved_", ctypes.c_int32)]
+                ("fused_remap", ctypes.c_int32), ("reserved_", ctypes.c_int32),
+                ("cold_rows", ctypes.c_int64 * MAX_MODES), ("cold_degree", ctypes.c_int64 * MAX_MODES)]
 
 
 class Timing(ctypes.Structure):
@@ -223,6 +224,7 @@ class Mttkrp:
             "shard_policy": "alg1" if raw.shard_policy else "equal", "kappa": raw.kappa, "fused_remap": bool(raw.fused_remap),
             "remap_plain_ms": list(raw.remap_plain_ms)[:n], "remap_twopass_ms": list(raw.remap_twopass_ms)[:n],
             "max_partition_nnz": list(raw.max_partition_nnz)[:n], "min_partition_nnz": list(raw.min_partition_nnz)[:n],
+            "cold_rows": list(raw.cold_rows)[:n], "cold_degree": list(raw.cold_degree)[:n],
         }
 
     def partition_rows(self, d: int, kappa: int):

@@ -382,6 +382,7 @@ mttkrp_status_t mttkrp_get_info(mttkrp_handle_t h, mttkrp_info_t* info) {
     info->remaps_done = h->remaps_done;
     for (int m = 0; m < h->N; ++m) { info->remap_plain_ms[m] = h->mode[m].plain_ms; info->remap_twopass_ms[m] = h->mode[m].twopass_ms; }
     info->fused_remap = h->fuse;
+    for (int m = 0; m < h->N; ++m) { info->cold_rows[m] = h->cold_rows[m]; info->cold_degree[m] = (int64_t)h->cold_deg[m]; }
     info->shard_policy = h->policy;
     info->kappa = h->kappa;
     for (int m = 0; m < h->N; ++m) { info->max_partition_nnz[m] = h->mode[m].max_bin; info->min_partition_nnz[m] = h->mode[m].min_bin; }

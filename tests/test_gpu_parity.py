@@ -416,6 +416,33 @@ def test_kernel_variants_all_entries(P, monkeypatch, deep):
         assert max(info["num_split_rows"]) > 0
 
 
+@pytest.mark.parametrize("keep", ["0", "7", "100"])
+def test_cold_row_prefetch_marks(P, monkeypatch, keep):
+    # The batch variant of the kernel requests "cold" factor rows (not among the MTTKRP_PREFETCH_ROWS most frequent
+    # of their factor matrix; marks in the spare bits of the record's key words) into L2 ahead of
+    # their gathers.  A small K puts marks on scaled tensors: the remapped copy must still be the oracle-sorted COO
+    # bit for bit (the marks never leak into indices) and every entry of every Y_d must match; the reported counts
+    # follow the documented rule (cold = degree below a threshold, at most K rows are not cold).
+    monkeypatch.setenv("MTTKRP_FORCE_DEEP", "1")
+    monkeypatch.setenv("MTTKRP_PREFETCH_ROWS", keep)
+    for dims, nnz in [((40, 30, 50), 3000), ((90, 70), 2500)]:
+        t = W.tiny_tensor(dims, nnz, seed=nnz)
+        for R in (16, 32):
+            _run_case(P, list(dims), t.idx, t.vals, R, seed=5)
+    spec = W.CONFIGS[2].scaled(300_137)
+    t = W.generate_tensor(spec)
+    worst, info = _run_case(P, spec.dims, t.idx, t.vals, 32, seed=6, order_modes=[0, 1, 2, 0, 2, 1])
+    K = int(keep)
+    for m in range(3):
+        deg = np.bincount(t.idx[m].numpy(), minlength=spec.dims[m])
+        if K == 0:
+            assert info["cold_rows"][m] == 0 and info["cold_degree"][m] == 0
+        else:
+            T = info["cold_degree"][m]
+            assert info["cold_rows"][m] == int((deg < T).sum())
+            assert spec.dims[m] - info["cold_rows"][m] <= K
+
+
 def test_calls_on_different_streams_are_ordered(P):
     # Calls on one handle share the tensor copies and the carry buffer.  The library orders them itself: a call
     # on another stream waits for the handle's previous work (include/mttkrp.h conventions), so issuing the modes
