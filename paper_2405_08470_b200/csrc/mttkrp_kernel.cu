@@ -448,22 +448,27 @@ __device__ __forceinline__ void shard_body(const KernelArgs<N>& a, const int64_t
             int stage = 0;
             for (int r = 0; r < nrounds; ++r) {
                 issue_round();                                // round r+AHEAD, reuses the stage of round r-1
-                cp_async_wait<AHEAD - 1>();                   // rounds <= r+1 have landed
+#ifndef MK_PF_DIST       // rounds between the L2 prefetch of a cold row and its gather (needs MK_STAGES >= MK_PF_DIST + 2)
+#define MK_PF_DIST 1
+#endif
+                static_assert(AHEAD >= MK_PF_DIST, "prefetch distance");
+                cp_async_wait<AHEAD - MK_PF_DIST>();          // rounds <= r+MK_PF_DIST have landed
                 __syncwarp();
                 const int nstage = (stage + 1 == STAGES) ? 0 : stage + 1;
                 const uint32_t cs = ring_gs + 4u * (uint32_t)(stage * STAGEW);
                 const uint32_t ns = ring_gs + 4u * (uint32_t)(nstage * STAGEW);
+                const uint32_t ps = ring_gs + 4u * (uint32_t)(((stage + MK_PF_DIST) % STAGES) * STAGEW);
 #if MK_PREFETCH
                 // Cold rows (common.cuh: outside the K most frequent of their factor matrix, so they almost always miss
                 // L2 when the factors overflow it) of the NEXT round are requested into L2 now, one round (~3000 clk)
                 // before their gathers; lane p of the group looks at record p of that round.  The batch then waits for
                 // L2 hits instead of HBM reads (configs[2]: -7 % per mode).
-                if (r + 1 < nrounds) {
+                if (r + MK_PF_DIST < nrounds) {
 #pragma unroll
                     for (int i = 0; i < (K + LPN - 1) / LPN; ++i) {
                         const int pr = sub + i * LPN;
                         if (K % LPN == 0 || pr < K) {
-                            const uint4 q = lds128(ns + 4u * (uint32_t)(pr * ROWW));
+                            const uint4 q = lds128(ps + 4u * (uint32_t)(pr * ROWW));
                             const uint32_t klast = N == 3 ? q.z : q.y;
                             if (q.x & kCold) prefetch_l2(reinterpret_cast<const float4*>(a.fac[N - 1]) + (size_t)klast * LPN);
                             if constexpr (N == 3) {
