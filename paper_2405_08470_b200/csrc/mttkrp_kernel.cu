@@ -95,10 +95,23 @@ __device__ __forceinline__ uint64_t l2_policy_evict_first() {
 #endif
 #define MK_STR2(x) #x
 #define MK_STR(x) MK_STR2(x)
+#ifndef MK_L1POL         // experiment: L1 eviction priority per LEVEL (uniform per instruction). 1: last level no_allocate;
+#define MK_L1POL 0       // 2: last level evict_first; 3: fiber level evict_last; 4: fiber evict_last + last evict_first;
+#endif                   // 5: fiber evict_last + last no_allocate
 __device__ __forceinline__ float4 ldg_pol(const float4* p, int kind) {   // kind 0: last level, 1: fiber level
-#if MK_ROWPOL == 0
+#if MK_ROWPOL == 0 && MK_L1POL == 0
     (void)kind;
     return __ldg(p);
+#elif MK_ROWPOL == 0
+    float4 v;
+    if (kind == 0 && (MK_L1POL == 1 || MK_L1POL == 5))
+        asm("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    else if (kind == 0 && (MK_L1POL == 2 || MK_L1POL == 4))
+        asm("ld.global.nc.L1::evict_first.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    else if (kind == 1 && MK_L1POL >= 3)
+        asm("ld.global.nc.L1::evict_last.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    else v = __ldg(p);
+    return v;
 #else
     float4 v;
     const bool last_pol = (MK_ROWPOL == 1 || MK_ROWPOL == 3), fiber_pol = (MK_ROWPOL == 1 || MK_ROWPOL == 2);

@@ -427,7 +427,7 @@ def test_cold_row_prefetch_marks(P, monkeypatch, keep):
     monkeypatch.setenv("MTTKRP_PREFETCH_ROWS", keep)
     for dims, nnz in [((40, 30, 50), 3000), ((90, 70), 2500)]:
         t = W.tiny_tensor(dims, nnz, seed=nnz)
-        for R in (16, 32):
+        for R in (8, 16, 32, 64):
             _run_case(P, list(dims), t.idx, t.vals, R, seed=5)
     spec = W.CONFIGS[2].scaled(300_137)
     t = W.generate_tensor(spec)
