@@ -399,10 +399,10 @@ __device__ __forceinline__ void shard_body(const KernelArgs<N>& a, const int64_t
             // ---- batch variant (N <= 3) -------------------------------------------------------------------------
             // ptxas tracks every factor-row LDG of this loop on ONE scoreboard, so any wait drains all gathers in
             // flight: a software pipeline degenerates into "issue, wait for everything, compute"
-            // (profiles/r2_scoreboards.md).  This variant makes that structure explicit and deep: the records of B = 4
+            // (profiles/r2_sass_hot_loop.md).  This variant makes that structure explicit and deep: the records of B = 4
             // steps are read with back-to-back LDS.128, their B last-level rows and up to B fiber rows are requested
             // together (up to 8 independent 128-bit gathers per lane in flight), then the B steps are computed.  Costs
-            // 64 registers (4 blocks per SM); one vote per batch replaces the per-step output-row-end test.
+            // 80 registers (3 blocks per SM); one vote per batch replaces the per-step output-row-end test.
 #ifndef MK_B
 #define MK_B 4
 #endif
