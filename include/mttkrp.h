@@ -174,6 +174,33 @@ mttkrp_status_t mttkrp_get_info(mttkrp_handle_t h, mttkrp_info_t* info /*host, o
 mttkrp_status_t mttkrp_get_perm(mttkrp_handle_t h, int d, uint32_t* perm_dev, uint32_t* scratch_dev,
                                 void* cuda_stream);
 
+/*
+ * mttkrp_get_perm without the caller's scratch buffer, for callers that cannot allocate device memory when they call.
+ *
+ * Who that is: code hosted by an application whose own memory pool has already taken the GPU's memory (a raw
+ * cudaMalloc there fails for lack of memory the pool is sitting on, and if it succeeds the pool's accounting no
+ * longer matches the device), and code on a multi-stream pipeline that cannot afford the device-wide stall that
+ * cudaMalloc and cudaFree bring.  mttkrp_get_perm asks such a caller for a second nnz-word buffer it has no way to
+ * produce.  Here that buffer is a fixed array inside the library image instead; the call itself uses no cudaMalloc,
+ * no cudaFree and no library routine that allocates.
+ *
+ *   perm_dev: device uint32 [nnz], the output, exactly as mttkrp_get_perm writes it (bit for bit).
+ *   Limit:    nnz <= MTTKRP_NOALLOC_MAX_NNZ (4,194,304 nonzeros; the array is 16 MiB).  A larger handle gets
+ *             MTTKRP_EUNSUPPORTED and nothing is launched; use mttkrp_get_perm for it.
+ *   Cost:     every GPU on which this library is loaded holds those 16 MiB until the process ends, used or not.
+ *   Set-up:   the first call on a device looks up the array's device address (once per device; the handle's device
+ *             must be current, else MTTKRP_EINVAL).  Make that first call before any stream capture begins.
+ *   Sharing:  all calls on one device use the same array.  Calls on the same stream are ordered and safe; two calls
+ *             that can overlap on the GPU (different streams without a dependency, different handles or host
+ *             threads) race on it and may return wrong permutations - serialise them yourself.  The array keeps
+ *             what the last call left in it; that is harmless, because every word a call reads it has written
+ *             first, so nothing needs to start at zero.
+ * Asynchronous on cuda_stream.  Errors: EINVAL (NULL handle / perm_dev, d out of range, wrong current device),
+ * EUNSUPPORTED (nnz over the limit, device ordinal >= 64), ECUDA.
+ */
+#define MTTKRP_NOALLOC_MAX_NNZ (1 << 22)
+mttkrp_status_t mttkrp_get_perm_noalloc(mttkrp_handle_t h, int d, uint32_t* perm_dev, void* cuda_stream);
+
 /* Copy the resident tensor copy out as SoA COO in its current layout order (device int32
  * [nmodes][nnz] in ORIGINAL mode numbering, device fp32 [nnz]).  Test hook for the remap. */
 mttkrp_status_t mttkrp_export_coo(mttkrp_handle_t h, int32_t* idx_dev, float* vals_dev, void* cuda_stream);

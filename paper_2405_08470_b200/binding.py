@@ -15,6 +15,7 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmttkrp_b200.so")
 MAX_MODES = 8
+NOALLOC_MAX_NNZ = 1 << 22          # MTTKRP_NOALLOC_MAX_NNZ in include/mttkrp.h
 
 OK, EINVAL, EINDEX, EUNSUPPORTED, EWORKSPACE, ECUDA = range(6)
 _STATUS_NAMES = {0: "MTTKRP_OK", 1: "MTTKRP_EINVAL", 2: "MTTKRP_EINDEX", 3: "MTTKRP_EUNSUPPORTED",
@@ -22,7 +23,7 @@ _STATUS_NAMES = {0: "MTTKRP_OK", 1: "MTTKRP_EINVAL", 2: "MTTKRP_EINDEX", 3: "MTT
 
 EXPORTS = ["mttkrp_workspace_bytes", "mttkrp_create", "mttkrp_mode", "mttkrp_sweep", "mttkrp_remap_to",
            "mttkrp_sweep_host", "mttkrp_destroy", "mttkrp_last_error", "mttkrp_get_info", "mttkrp_get_perm",
-           "mttkrp_export_coo", "mttkrp_timing_begin", "mttkrp_timing_end", "mttkrp_partition_rows", "mttkrp_version"]
+           "mttkrp_get_perm_noalloc", "mttkrp_export_coo", "mttkrp_timing_begin", "mttkrp_timing_end", "mttkrp_partition_rows", "mttkrp_version"]
 
 
 class MttkrpError(RuntimeError):
@@ -76,6 +77,7 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.mttkrp_destroy.argtypes = [vp]
     lib.mttkrp_get_info.argtypes = [vp, ctypes.POINTER(Info)]
     lib.mttkrp_get_perm.argtypes = [vp, ctypes.c_int, vp, vp, vp]
+    lib.mttkrp_get_perm_noalloc.argtypes = [vp, ctypes.c_int, vp, vp]
     lib.mttkrp_export_coo.argtypes = [vp, vp, vp, vp]
     lib.mttkrp_partition_rows.argtypes = [vp, ctypes.c_int, ctypes.c_int, vp, vp, vp, vp]
     lib.mttkrp_timing_begin.argtypes = [vp]
@@ -244,6 +246,21 @@ class Mttkrp:
         with torch.cuda.device(self.device):
             _check(load_library().mttkrp_get_perm(self._h, int(d), perm.data_ptr(), scratch.data_ptr(), _stream()))
         return perm[: self.nnz]
+
+    def get_perm_noalloc(self, d: int, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+        """`get_perm` for callers that cannot allocate device memory at call time (all of the GPU's memory already
+        belongs to the host application's pool, or cudaMalloc's device-wide stall is not acceptable): the second
+        buffer `get_perm` allocates is a fixed 16 MiB array inside the library instead.  Pass a preallocated int32
+        `out` of nnz elements and this method allocates nothing on the device either.  Handles with more than
+        NOALLOC_MAX_NNZ nonzeros raise MTTKRP_EUNSUPPORTED.  All calls on a device share the array: do not let two
+        of them overlap on the GPU."""
+        if out is None:
+            out = torch.empty(max(self.nnz, 1), dtype=torch.int32, device=self.device)
+        elif not out.is_cuda or out.dtype != torch.int32 or not out.is_contiguous() or out.numel() < self.nnz:
+            raise ValueError("out must be a contiguous int32 CUDA tensor with at least nnz elements")
+        with torch.cuda.device(self.device):
+            _check(load_library().mttkrp_get_perm_noalloc(self._h, int(d), out.data_ptr(), _stream()))
+        return out[: self.nnz]
 
     def export_coo(self):
         idx = torch.empty((self.nmodes, max(self.nnz, 1)), dtype=torch.int32, device=self.device)[:, : self.nnz].contiguous()

@@ -16,7 +16,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 OBJDIR = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libmttkrp_b200.so")
-SOURCES = ["api.cu", "build.cu", "remap.cu", "mttkrp_kernel.cu"]
+SOURCES = ["api.cu", "build.cu", "remap.cu", "mttkrp_kernel.cu", "noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--use_fast_math=false", "-I", INCLUDE]
 
