@@ -28,14 +28,29 @@
  *   - Calls on one handle execute in call order even when they are given different streams: the handle
  *     remembers the stream of its last call and makes a call on another stream wait (cudaStreamWaitEvent) for
  *     the work launched before it.  The caller still orders its own use of `out` and of the factor buffers.
- *   - Process environment variables read by mttkrp_workspace_bytes / mttkrp_create (test and experiment knobs;
- *     unset = the library decides): MTTKRP_KEY_ORDER = revcyclic|desc|asc|cyclic (anything else: EINVAL),
- *     MTTKRP_PACK = 0|1, MTTKRP_REMAP_BLOCKED = 0|1, MTTKRP_REMAP_BLOCK_LOG2 (clamped to [10,26]),
- *     MTTKRP_REMAP_TWOPASS = 0|1, MTTKRP_TWOPASS_WINDOW_LOG2 (clamped to [8,26]),
- *     MTTKRP_FORCE_DEEP = 0|1 (kernel variant), MTTKRP_PREFETCH_ROWS (rows per factor matrix that are NOT prefetched
- *     into L2, default 65536; 0 = no prefetch), MTTKRP_FUSE = 0|1 (remap inside the MTTKRP kernel), MTTKRP_SHARD_POLICY = equal|alg1 and MTTKRP_KAPPA (number of
- *     partitions of the paper's Alg. 1 policy, default one per SM).  They must not change between the size query
- *     and create.
+ *   - Process environment variables (test and experiment knobs; unset = the library decides).  They are read in one
+ *     place, by mttkrp_workspace_bytes and mttkrp_create, and checked BEFORE anything is launched: a malformed value
+ *     is MTTKRP_EINVAL with the variable named in mttkrp_last_error(), never a silent default.  0|1 switches accept
+ *     exactly "0" or "1"; numbers are decimal integers with nothing after them.  The handle keeps the values it was
+ *     created with; they must not change between the size query and create.
+ *       MTTKRP_KEY_ORDER = revcyclic|desc|asc|cyclic      sort-key order of the layouts
+ *       MTTKRP_PACK = 0|1                                 0: 4*(nmodes+1)-byte records even where 16-byte packing fits
+ *       MTTKRP_REMAP_BLOCKED = 0|1                        pin the blocked remap walk off / on for every transition
+ *       MTTKRP_REMAP_BLOCK_LOG2 = integer                 log2 records per source block, clamped to [10,26]
+ *       MTTKRP_REMAP_TWOPASS = 0|1                        pin the two-pass remap walk off / on.  Unpinned, create
+ *                                                         TIMES both walks on the real tensor (median of 3 runs each)
+ *                                                         and keeps the faster per transition, so on a busy GPU the
+ *                                                         choice in info.remap_blocked can differ between runs (the
+ *                                                         results never do); pin it for reproducible timings
+ *       MTTKRP_TWOPASS_WINDOW_LOG2 = integer              log2 records per destination window, clamped to [8,26]
+ *       MTTKRP_FORCE_DEEP = 0|1                           pin the MTTKRP kernel variant (nmodes <= 3)
+ *       MTTKRP_PREFETCH_ROWS = integer >= 0               rows per factor matrix that are NOT prefetched into L2
+ *                                                         (default 65536; 0 = no prefetch)
+ *       MTTKRP_FUSE = 0|1                                 1: the remap runs inside the MTTKRP kernel.  Needs 16-byte
+ *                                                         records (nmodes == 3, or packed nmodes >= 4) and the default
+ *                                                         shard policy; asked for elsewhere it is MTTKRP_EUNSUPPORTED
+ *       MTTKRP_SHARD_POLICY = equal|alg1                  alg1: the paper's Alg. 1 partitioner
+ *       MTTKRP_KAPPA = integer in [1,65536]               partitions of the alg1 policy (default one per SM)
  */
 #ifndef MTTKRP_B200_H
 #define MTTKRP_B200_H
@@ -90,8 +105,8 @@ typedef struct {
     int32_t kappa;                       /* partitions of the Alg. 1 policy (0 under the default policy) */
     int64_t max_partition_nnz[MTTKRP_MAX_MODES];   /* Alg. 1 policy: largest / smallest partition per mode, in nonzeros */
     int64_t min_partition_nnz[MTTKRP_MAX_MODES];
-    double remap_plain_ms[MTTKRP_MAX_MODES];       /* create-time measurement of the plain and of the two-pass walk of */
-    double remap_twopass_ms[MTTKRP_MAX_MODES];     /* that transition on this tensor (0: two passes were not a candidate) */
+    double remap_plain_ms[MTTKRP_MAX_MODES];       /* create-time measurement (median of 3 runs) of the plain and of the two-pass */
+    double remap_twopass_ms[MTTKRP_MAX_MODES];     /* walk of that transition on this tensor (0: two passes were not a candidate) */
     int32_t fused_remap;                 /* 1: MTTKRP_FUSE=1 is in effect - the MTTKRP kernel of mode d also scatters the
                                             records into the layout of mode (d+1)%N (Alg. 4 lines 15-19) */
     int32_t reserved_;

@@ -177,10 +177,8 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
     h->max_rank = max_rank;
     h->device = dev;
     h->num_sms = num_sms;
-    {
-        const char* env = getenv("MTTKRP_FORCE_DEEP");               // tests: 0 / 1 pins the kernel variant
-        h->force_deep = env ? (env[0] == '1' ? 1 : 0) : -1;
-    }
+    h->knobs = lp.knobs;
+    h->force_deep = lp.knobs.force_deep;                          // tests: 0 / 1 pins the kernel variant
     h->jump[0] = reinterpret_cast<uint32_t*>(ws + p.jump[0]);
     h->jump[1] = reinterpret_cast<uint32_t*>(ws + p.jump[1]);
     h->jump_map = nullptr;

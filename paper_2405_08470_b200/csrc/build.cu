@@ -3,6 +3,7 @@
 // PAPER.md:185; unique per element, Observation 1 PAPER.md:297-299), the mode-0 tensor copy
 // (PAPER.md:145), and per-mode tables (empty output rows; rows that span shards).
 // The paper builds its format on the CPU (Sec. 5.7); here it is done on the GPU.
+#include <cerrno>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -543,28 +544,78 @@ void choose_key_order(int N, const int64_t* dims, int d, const char* env, int* o
     for (int j = 0; j < n; ++j) order[j + 1] = rest[j];
 }
 
+// ---- environment knobs ---------------------------------------------------------------------------------------
+// 0/1 switches accept exactly "0" or "1"; integers must be decimal numbers with nothing after them.
+static mttkrp_status_t env_flag(const char* name, int* out) {
+    *out = -1;
+    const char* e = getenv(name);
+    if (!e) return MTTKRP_OK;
+    if ((e[0] == '0' || e[0] == '1') && e[1] == '\0') { *out = e[0] - '0'; return MTTKRP_OK; }
+    set_error("%s=%s is not 0 or 1", name, e);
+    return MTTKRP_EINVAL;
+}
+static mttkrp_status_t env_int(const char* name, long long lo, long long hi, bool clamp, long long unset, long long* out) {
+    *out = unset;
+    const char* e = getenv(name);
+    if (!e) return MTTKRP_OK;
+    char* end = nullptr;
+    errno = 0;
+    const long long v = strtoll(e, &end, 10);
+    if (end == e || *end != '\0' || errno != 0) { set_error("%s=%s is not an integer", name, e); return MTTKRP_EINVAL; }
+    if (v < lo || v > hi) {
+        if (!clamp) { set_error("%s=%s outside [%lld, %lld]", name, e, lo, hi); return MTTKRP_EINVAL; }
+        *out = v < lo ? lo : hi;
+        return MTTKRP_OK;
+    }
+    *out = v;
+    return MTTKRP_OK;
+}
+
+mttkrp_status_t read_knobs(Knobs* k) {
+    memset(k, 0, sizeof(*k));
+    if (const char* e = getenv("MTTKRP_KEY_ORDER")) {
+        if (!known_key_order(e)) { set_error("MTTKRP_KEY_ORDER=%s is not one of revcyclic, desc, asc, cyclic", e); return MTTKRP_EINVAL; }
+        snprintf(k->key_order, sizeof(k->key_order), "%s", e);
+    }
+    long long v = 0;
+    MK_TRY(env_flag("MTTKRP_PACK", &k->pack));                       // 0 forces 4*(N+1)-byte records (tests)
+    MK_TRY(env_flag("MTTKRP_REMAP_BLOCKED", &k->remap_blocked));     // 0 / 1 force the walk (experiments)
+    MK_TRY(env_flag("MTTKRP_REMAP_TWOPASS", &k->remap_twopass));     // 0 / 1 force the walk (tests, experiments)
+    MK_TRY(env_flag("MTTKRP_FORCE_DEEP", &k->force_deep));           // 0 / 1 pins the kernel variant (tests)
+    MK_TRY(env_flag("MTTKRP_FUSE", &k->fuse));                       // 1: Alg. 3 runs inside the MTTKRP kernel
+    MK_TRY(env_int("MTTKRP_REMAP_BLOCK_LOG2", 10, 26, true, -1, &v));    k->remap_block_log2 = (int)v;
+    MK_TRY(env_int("MTTKRP_TWOPASS_WINDOW_LOG2", 8, 26, true, -1, &v));  k->twopass_window_log2 = (int)v;
+    MK_TRY(env_int("MTTKRP_PREFETCH_ROWS", 0, (1ll << 40), false, -1, &v)); k->prefetch_rows = v;
+    MK_TRY(env_int("MTTKRP_KAPPA", 1, 65536, false, 0, &v));             k->kappa = (int)v;
+    if (const char* pol = getenv("MTTKRP_SHARD_POLICY")) {           // equal (default) | alg1 (the paper's partitioner)
+        if (strcmp(pol, "equal") != 0 && strcmp(pol, "alg1") != 0) {
+            set_error("MTTKRP_SHARD_POLICY=%s is not one of equal, alg1", pol);
+            return MTTKRP_EINVAL;
+        }
+        k->policy = strcmp(pol, "alg1") == 0 ? 1 : 0;
+    }
+    return MTTKRP_OK;
+}
+
 mttkrp_status_t plan_layouts(int N, const int64_t* dims, int64_t nnz, LayoutPlan* lp) {
+    memset(lp, 0, sizeof(*lp));
+    MK_TRY(read_knobs(&lp->knobs));
+    const Knobs& kn = lp->knobs;
     // Key order of the layouts (reading 4).  The default makes every remap a stable partition
     // by one key, which the blocked remap turns into L2-resident gathers; that pays when the nonzeros a
     // source block sends to one output row form runs of several records.  The expected run for mode d
     // is nnz / (dims[d] * number of blocks); when most modes are too large for that, the size-ordered
     // tuple (one remap of the cycle moves whole fibers) is the better choice.
-    const char* order_env = getenv("MTTKRP_KEY_ORDER");
-    if (order_env && !known_key_order(order_env)) {
-        set_error("MTTKRP_KEY_ORDER=%s is not one of revcyclic, desc, asc, cyclic", order_env);
-        return MTTKRP_EINVAL;
-    }
+    const char* order_env = kn.key_order[0] ? kn.key_order : nullptr;
     if (!order_env) {
         const double nblk = (double)((nnz >> 20) > 0 ? (nnz >> 20) : 1);
         int good = 0;
         for (int d = 0; d < N; ++d) good += ((double)nnz / ((double)dims[d] * nblk) >= 1.0) ? 1 : 0;
         order_env = (2 * good >= N) ? "revcyclic" : "desc";
     }
-    memset(lp, 0, sizeof(*lp));
     for (int d = 0; d < N; ++d) choose_key_order(N, dims, d, order_env, lp->order[d]);
     // Record format: packed 16-byte records for N >= 4 when every layout fits (common.cuh PackDesc).
-    const char* pack_env = getenv("MTTKRP_PACK");                 // 0 forces 4*(N+1)-byte records (tests)
-    bool packed = N >= 4 && !(pack_env && pack_env[0] == '0');
+    bool packed = N >= 4 && kn.pack != 0;
     for (int d = 0; d < N && packed; ++d) {
         int off = 0;
         for (int l = 0; l < N; ++l) {
@@ -577,17 +628,20 @@ mttkrp_status_t plan_layouts(int N, const int64_t* dims, int64_t nnz, LayoutPlan
     }
     lp->packed = packed ? 1 : 0;
     lp->rec_words = packed ? 4 : N + 1;
-    const char* pol = getenv("MTTKRP_SHARD_POLICY");              // equal (default) | alg1 (the paper's partitioner)
-    if (pol && strcmp(pol, "equal") != 0 && strcmp(pol, "alg1") != 0) {
-        set_error("MTTKRP_SHARD_POLICY=%s is not one of equal, alg1", pol);
-        return MTTKRP_EINVAL;
+    lp->policy = kn.policy;
+    lp->kappa = kn.kappa;
+    // The fused kernel exists for 16-byte records under the default shard policy; asking for it where it cannot
+    // run is an error the caller sees, not a request that is dropped.
+    lp->fuse = 0;
+    if (kn.fuse == 1) {
+        if (lp->rec_words != 4) {
+            set_error("MTTKRP_FUSE=1 needs 16-byte records (nmodes == 3, or nmodes >= 4 with packed records); this tensor has %d-byte records",
+                      4 * lp->rec_words);
+            return MTTKRP_EUNSUPPORTED;
+        }
+        if (lp->policy != 0) { set_error("MTTKRP_FUSE=1 cannot be combined with MTTKRP_SHARD_POLICY=alg1"); return MTTKRP_EUNSUPPORTED; }
+        lp->fuse = 1;
     }
-    lp->policy = (pol && strcmp(pol, "alg1") == 0) ? 1 : 0;
-    const char* fuse = getenv("MTTKRP_FUSE");                     // 1: Alg. 3 runs inside the MTTKRP kernel (16-byte records)
-    lp->fuse = (fuse && fuse[0] == '1' && lp->rec_words == 4 && lp->policy == 0) ? 1 : 0;
-    const char* kap = getenv("MTTKRP_KAPPA");
-    lp->kappa = kap ? atoi(kap) : 0;
-    if (lp->kappa < 0 || lp->kappa > 65536) { set_error("MTTKRP_KAPPA=%s outside [1, 65536]", kap); return MTTKRP_EINVAL; }
     return MTTKRP_OK;
 }
 
@@ -639,8 +693,7 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
     // Cold-row marks (common.cuh; unpacked records, N <= 3): degree of every index of every mode, and per mode the
     // degree below which a row is not among the K = MTTKRP_PREFETCH_ROWS most frequent ones (0 switches the marks off).
     for (int m = 0; m < N; ++m) { h->cold_deg[m] = 0; h->cold_rows[m] = 0; }
-    int64_t k_keep = 65536;
-    if (const char* e = getenv("MTTKRP_PREFETCH_ROWS")) k_keep = std::max<long long>(0, atoll(e));
+    const int64_t k_keep = h->knobs.prefetch_rows >= 0 ? h->knobs.prefetch_rows : 65536;
     const bool marks = nnz > 0 && N <= 3 && !h->packed && k_keep > 0;
     if (marks) {
         uint32_t hh[kDegBins];
@@ -806,14 +859,8 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
         // Blocked remap order (remap.cu): destination positions of the remap d -> d+1 grouped, stably,
         // by the source block they read from: one 8-bit radix pass on the block id.  The block is sized
         // to stay L2-resident while the whole grid gathers from it.
-        int block_log2 = 20;
-        {
-            const char* env = getenv("MTTKRP_REMAP_BLOCK_LOG2");
-            if (env) block_log2 = atoi(env);
-            if (block_log2 < 10) block_log2 = 10;
-            if (block_log2 > 26) block_log2 = 26;                     // 2^26 records = 1 GB windows: far beyond any L2
-            while ((nnz >> block_log2) > 255) ++block_log2;            // at most 256 blocks (one radix digit)
-        }
+        int block_log2 = h->knobs.remap_block_log2 >= 0 ? h->knobs.remap_block_log2 : 20;   // knob clamped to [10,26]
+        while ((nnz >> block_log2) > 255) ++block_log2;                // at most 256 blocks (one radix digit)
         for (int d = 0; d < N; ++d) {
             ModeMeta& mm = h->mode[d];
             mm.block_log2 = block_log2;
@@ -833,7 +880,7 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
     MK_CUDA(cudaMemcpyAsync(counts, small + 8, sizeof(uint32_t) * 2 * N, cudaMemcpyDeviceToHost, st));
     MK_CUDA(cudaMemcpyAsync(breaks, small + 32, sizeof(uint32_t) * 2 * kMaxModes, cudaMemcpyDeviceToHost, st));
     MK_CUDA(cudaStreamSynchronize(st));
-    const char* benv = getenv("MTTKRP_REMAP_BLOCKED");           // 0 / 1 force the choice (experiments)
+    const int benv = h->knobs.remap_blocked;                     // 0 / 1 force the choice (experiments), -1: decide here
     for (int d = 0; d < N; ++d) {
         h->mode[d].n_chains = (nnz > 0 && h->policy == 0) ? counts[2 * d] : 0;   // Alg. 1 policy: no row spans blocks
         h->mode[d].n_empty = nnz > 0 ? counts[2 * d + 1] : h->dims[d];
@@ -846,21 +893,20 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
         const bool fits = ((int64_t)h->rec_words * 4 << h->mode[d].block_log2) <= (48ll << 20);
         bool blocked = nnz > 0 && fits && (nnz >> h->mode[d].block_log2) >= 2 && nnz / runs >= 4 &&
                        (double)nnz / (double)src_runs < 1.5;
-        if (benv) blocked = nnz > 0 && benv[0] == '1';
+        if (benv >= 0) blocked = nnz > 0 && benv == 1;
         h->mode[d].blocked = blocked ? 1 : 0;
         h->mode[d].avg_run = nnz > 0 ? (double)nnz / (double)runs : 0.0;
         h->mode[d].plain_ms = h->mode[d].twopass_ms = 0.f;
     }
     // Two-pass remap for the transitions that stay a random gather (16-byte records, tensors of many windows): build
-    // the two maps into the (otherwise unused) ord / osrc arrays, then TIME one cycle of transitions with the plain
-    // walk and one with the two passes on the real tensor and keep, per transition, the faster one.
-    const char* tenv = getenv("MTTKRP_REMAP_TWOPASS");          // 0 / 1 force the choice (tests, experiments)
-    const bool tp_forced_on = tenv && tenv[0] == '1', tp_forced_off = (tenv && tenv[0] == '0') || benv;
+    // the two maps into the (otherwise unused) ord / osrc arrays, then TIME cycles of transitions with the plain
+    // walk and with the two passes on the real tensor and keep, per transition, the faster one (medians, below).
+    const int tenv = h->knobs.remap_twopass;                    // 0 / 1 force the choice (tests, experiments)
+    const bool tp_forced_on = tenv == 1, tp_forced_off = tenv == 0 || benv >= 0;
     bool cand[kMaxModes] = {false};
     bool any_cand = false;
     if (nnz > 0 && h->rec_words == 4 && !tp_forced_off) {
-        int wlog = kTwoPassWindowLog2;
-        if (const char* wenv = getenv("MTTKRP_TWOPASS_WINDOW_LOG2")) wlog = std::min(26, std::max(8, atoi(wenv)));   // tests
+        int wlog = h->knobs.twopass_window_log2 >= 0 ? h->knobs.twopass_window_log2 : kTwoPassWindowLog2;   // knob: tests
         while ((nnz >> wlog) > 255) ++wlog;
         for (int d = 0; d < N; ++d) {
             const int64_t src_runs = (int64_t)breaks[kMaxModes + d] + 1;
@@ -885,26 +931,38 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
         MK_CUDA(cudaGetLastError());
     }
     if (any_cand) {
-        cudaEvent_t e0, e1;
-        MK_CUDA(cudaEventCreate(&e0));
-        MK_CUDA(cudaEventCreate(&e1));
-        for (int pass = 0; pass < 3; ++pass) {                  // warm-up cycle, plain cycle, two-pass cycle
+        // One warm-up cycle, then kReps plain cycles and kReps two-pass cycles, alternating; per transition the MEDIAN
+        // of each walk decides (one sample per walk let a single disturbed run flip the choice).  The events are
+        // destroyed on every exit path; a failing create deletes the handle, so `blocked` needs no restoring there.
+        struct EventPair {
+            cudaEvent_t a = nullptr, b = nullptr;
+            ~EventPair() { if (a) cudaEventDestroy(a); if (b) cudaEventDestroy(b); }
+        } ev;
+        MK_CUDA(cudaEventCreate(&ev.a));
+        MK_CUDA(cudaEventCreate(&ev.b));
+        constexpr int kReps = 3;
+        int keep[kMaxModes];
+        float t_plain[kMaxModes][kReps], t_two[kMaxModes][kReps];
+        for (int d = 0; d < N; ++d) keep[d] = h->mode[d].blocked == 1 ? 1 : 0;
+        for (int cyc = 0; cyc < 1 + 2 * kReps; ++cyc) {
+            const bool two = cyc > 0 && cyc % 2 == 0;           // cycles 1, 3, 5 plain; 2, 4, 6 two passes
             for (int d = 0; d < N; ++d) {
-                h->mode[d].blocked = (pass == 2 && cand[d]) ? 2 : (h->mode[d].blocked == 1 ? 1 : 0);
-                MK_CUDA(cudaEventRecord(e0, st));
+                h->mode[d].blocked = (two && cand[d]) ? 2 : keep[d];
+                MK_CUDA(cudaEventRecord(ev.a, st));
                 MK_TRY(launch_remap(h, d, (d + 1) % N, nullptr, st));
-                MK_CUDA(cudaEventRecord(e1, st));
-                MK_CUDA(cudaEventSynchronize(e1));
+                MK_CUDA(cudaEventRecord(ev.b, st));
+                MK_CUDA(cudaEventSynchronize(ev.b));
                 float ms = 0.f;
-                MK_CUDA(cudaEventElapsedTime(&ms, e0, e1));
-                if (pass == 1) h->mode[d].plain_ms = cand[d] ? ms : 0.f;
-                if (pass == 2) h->mode[d].twopass_ms = cand[d] ? ms : 0.f;
+                MK_CUDA(cudaEventElapsedTime(&ms, ev.a, ev.b));
+                if (cyc > 0) (two ? t_two : t_plain)[d][(cyc - 1) / 2] = ms;
             }
         }
-        cudaEventDestroy(e0);
-        cudaEventDestroy(e1);
+        auto median3 = [](const float* t) { return std::max(std::min(t[0], t[1]), std::min(std::max(t[0], t[1]), t[2])); };
         for (int d = 0; d < N; ++d) {
+            h->mode[d].blocked = keep[d];
             if (!cand[d]) continue;
+            h->mode[d].plain_ms = median3(t_plain[d]);
+            h->mode[d].twopass_ms = median3(t_two[d]);
             h->mode[d].blocked = (tp_forced_on || h->mode[d].twopass_ms < 0.95f * h->mode[d].plain_ms) ? 2 : 0;
         }
         h->remaps_done = 0;                                      // the tensor is back in the mode-0 layout (N transitions per cycle)

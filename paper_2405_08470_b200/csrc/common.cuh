@@ -105,6 +105,23 @@ struct FuseArgs {
     PackDesc dd;                  // packed records: bit layout of the next layout
 };
 
+// Test and experiment knobs (include/mttkrp.h, "Process environment variables").  The environment is read in ONE place,
+// read_knobs (build.cu), by mttkrp_workspace_bytes and mttkrp_create before anything is launched; every value is
+// checked there (a malformed one is MTTKRP_EINVAL, not a silent default) and the handle keeps the parsed copy.
+struct Knobs {
+    char key_order[16];           // MTTKRP_KEY_ORDER, "" = the library decides
+    int pack;                     // MTTKRP_PACK: -1 unset / 0 / 1
+    int remap_blocked;            // MTTKRP_REMAP_BLOCKED: -1 / 0 / 1
+    int remap_block_log2;         // MTTKRP_REMAP_BLOCK_LOG2 clamped to [10,26], -1 unset
+    int remap_twopass;            // MTTKRP_REMAP_TWOPASS: -1 / 0 / 1
+    int twopass_window_log2;      // MTTKRP_TWOPASS_WINDOW_LOG2 clamped to [8,26], -1 unset
+    int force_deep;               // MTTKRP_FORCE_DEEP: -1 / 0 / 1
+    int64_t prefetch_rows;        // MTTKRP_PREFETCH_ROWS >= 0, -1 unset
+    int fuse;                     // MTTKRP_FUSE: -1 / 0 / 1
+    int policy;                   // MTTKRP_SHARD_POLICY: 0 equal (default), 1 alg1
+    int kappa;                    // MTTKRP_KAPPA in [1,65536], 0 unset (one partition per SM)
+};
+
 // Per-mode tables built by mttkrp_create.
 struct ModeMeta {
     int order[kMaxModes];     // sort-key order of this layout, order[0] == mode
@@ -189,6 +206,7 @@ struct mttkrp_handle_s {
     int device;
     int num_sms;              // SM count of `device` (grid sizing)
     int force_deep;           // MTTKRP_FORCE_DEEP at create: -1 = by factor size (default), 0 / 1 = never / always
+    mk::Knobs knobs;          // the environment as mttkrp_create read it
     uint32_t cold_deg[mk::kMaxModes];   // cold-row marks: a row of mode m is cold when its index occurs fewer than this many times (0: none)
     int64_t cold_rows[mk::kMaxModes];   // ... and how many rows of the mode that makes
     cudaStream_t last_stream; // stream of the last call that launched work for this handle
@@ -222,8 +240,10 @@ struct LayoutPlan {
     int fuse;                // MTTKRP_FUSE=1 and 16-byte records and the default shard policy
     int policy;              // MTTKRP_SHARD_POLICY: 0 equal (default), 1 alg1
     int kappa;               // MTTKRP_KAPPA (alg1): 0 = one partition per SM
+    Knobs knobs;             // every MTTKRP_* variable, parsed and checked
 };
-mttkrp_status_t plan_layouts(int N, const int64_t* dims, int64_t nnz, LayoutPlan* lp);   // EINVAL: bad MTTKRP_* override
+mttkrp_status_t read_knobs(Knobs* k);                                                    // EINVAL: malformed MTTKRP_* value
+mttkrp_status_t plan_layouts(int N, const int64_t* dims, int64_t nnz, LayoutPlan* lp);   // EINVAL / EUNSUPPORTED: bad MTTKRP_* override
 mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_rank, int rec_words, int num_sms, int kappa,
                                int fuse, WorkspacePlan* p);
 // Alg. 1 (reading 3): rows by descending degree (ties: lower index), each to the least-loaded

@@ -76,6 +76,53 @@ def test_environment_overrides_are_validated(lib, monkeypatch):
         assert P.mttkrp_workspace_bytes([1000, 800, 600], 100_000) > 0
 
 
+@pytest.mark.parametrize("name,bad,good", [
+    ("MTTKRP_PACK", ["yes", "2", "", "01", "1 "], ["0", "1"]),
+    ("MTTKRP_REMAP_BLOCKED", ["true", "-1", "10"], ["0", "1"]),
+    ("MTTKRP_REMAP_TWOPASS", ["on", "2"], ["0", "1"]),
+    ("MTTKRP_FORCE_DEEP", ["deep", "11"], ["0", "1"]),
+    ("MTTKRP_FUSE", ["fuse", "1x"], ["0", "1"]),
+    ("MTTKRP_REMAP_BLOCK_LOG2", ["big", "12.5", ""], ["12", "3", "99"]),          # numbers are clamped to [10, 26]
+    ("MTTKRP_TWOPASS_WINDOW_LOG2", ["x", "1e3"], ["11", "0", "40"]),              # clamped to [8, 26]
+    ("MTTKRP_PREFETCH_ROWS", ["many", "-1", "7 rows"], ["0", "7", "65536"]),
+    ("MTTKRP_KAPPA", ["0", "-3", "65537", "kappa", "12abc", ""], ["1", "148", "65536"]),
+    ("MTTKRP_SHARD_POLICY", ["alg2", ""], ["equal", "alg1"]),
+])
+def test_every_environment_knob_is_parsed_strictly(lib, monkeypatch, name, bad, good):
+    # A malformed value is an error before any launch (the size query runs the same parser as create), never a
+    # silent default; the message names the variable.
+    import paper_2405_08470_b200 as P
+    for v in bad:
+        monkeypatch.setenv(name, v)
+        with pytest.raises(P.MttkrpError) as e:
+            P.mttkrp_workspace_bytes([1000, 800, 600], 100_000)
+        assert e.value.status == 1 and name in str(e.value), (name, v)
+    for v in good:
+        monkeypatch.setenv(name, v)
+        assert P.mttkrp_workspace_bytes([1000, 800, 600], 100_000) > 0, (name, v)
+
+
+def test_fuse_request_that_cannot_apply_is_refused(lib, monkeypatch):
+    # MTTKRP_FUSE=1 exists for 16-byte records under the default shard policy.  Where it cannot run the caller is
+    # told (EUNSUPPORTED with the reason) instead of getting the unfused path without a word.
+    import paper_2405_08470_b200 as P
+    monkeypatch.setenv("MTTKRP_FUSE", "1")
+    assert P.mttkrp_workspace_bytes([1000, 800, 600], 100_000) > 0               # 3 modes: 16-byte records
+    assert P.mttkrp_workspace_bytes([100, 80, 60, 40], 100_000) > 0              # 4 modes, packed
+    with pytest.raises(P.MttkrpError) as e:
+        P.mttkrp_workspace_bytes([1000, 800], 100_000)                           # 2 modes: 12-byte records
+    assert e.value.status == 3 and "MTTKRP_FUSE" in str(e.value)
+    monkeypatch.setenv("MTTKRP_PACK", "0")
+    with pytest.raises(P.MttkrpError) as e:
+        P.mttkrp_workspace_bytes([100, 80, 60, 40], 100_000)                     # 4 modes, unpacked: 20-byte records
+    assert e.value.status == 3 and "16-byte" in str(e.value)
+    monkeypatch.delenv("MTTKRP_PACK")
+    monkeypatch.setenv("MTTKRP_SHARD_POLICY", "alg1")
+    with pytest.raises(P.MttkrpError) as e:
+        P.mttkrp_workspace_bytes([1000, 800, 600], 100_000)
+    assert e.value.status == 3 and "alg1" in str(e.value)
+
+
 def test_null_arguments_return_status_not_crash(lib):
     out = ctypes.c_void_p(None)
     dims = (ctypes.c_int64 * 3)(5, 4, 3)
