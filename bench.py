@@ -322,11 +322,59 @@ class Case:
                if tm["mttkrp_ms"] else None}
         return k_ms, alg, achieved, brk
 
+    def rows_gathered_per_nnz(self):
+        """Factor rows the kernel gathers per nonzero, per mode, counted from the resident tensor copy itself (measurement
+        code: torch ops on the exported COO, not part of the timed path).  In the mode-d layout the last key's row is
+        gathered for every nonzero and the row of level l (1 <= l <= N-2) once per run of equal (k_0..k_l) - the fiber
+        factoring of DESIGN.md Sec. 6."""
+        import torch
+        out = []
+        for d in range(self.N):
+            self.h.remap_to(d)
+            idx, _ = self.h.export_coo()
+            order = self.info["key_order"][d]
+            rows = float(self.nnz)
+            neq = torch.zeros(max(self.nnz - 1, 0), dtype=torch.bool, device=self.dev)
+            for l in range(self.N - 1):
+                neq |= idx[order[l], 1:] != idx[order[l], :-1]
+                if l >= 1:
+                    rows += float(neq.sum().item()) + 1.0
+            out.append(rows / max(self.nnz, 1))
+            del idx, neq
+        torch.cuda.empty_cache()
+        return out
+
     def close(self):
         import torch
         self.h.destroy()
         self.fac = self.outs = None
         torch.cuda.empty_cache()
+
+
+# L1-data-pipe model of the gather (DESIGN.md Sec. 6, probes A/F in profiles/r2_probes.md): an SM's L1 data pipe moves
+# one 128-byte wavefront per clock; a gathered 128-byte row costs ~1.0 pipe cycle on an L1 hit and ~1.5 when it comes from
+# L2; reading the 16-byte record costs >= 0.5.  The floor below charges every row the L2 price (rows that hit L1 make
+# the true floor lower, rows that miss L2 are not a pipe cost), so it is a model, not a bound that was measured tight.
+PIPE_CYCLES_PER_ROW_L2 = 1.5
+PIPE_CYCLES_PER_RECORD = 0.5
+
+
+def pipe_ceilings(rows_per_nnz, nnz, R, k_ms, sm_count, sm_mhz, traffic_bytes):
+    clk = sm_mhz * 1e6
+    wavefronts_per_row = max(1.0, R * 4 / 128.0)
+    rows = sum(rows_per_nnz) / len(rows_per_nnz)
+    cycles = rows * wavefronts_per_row * PIPE_CYCLES_PER_ROW_L2 + PIPE_CYCLES_PER_RECORD
+    floor_ms = nnz * cycles / (sm_count * clk) * 1e3
+    return {"l1_lines_gnnz_s": sm_count * clk / wavefronts_per_row / 1e9,
+            "rows_gathered_per_nnz": [round(x, 4) for x in rows_per_nnz],
+            "pipe_cycles_per_nnz": cycles, "pipe_floor_ms": floor_ms,
+            "frac_of_pipe_floor": floor_ms / k_ms if k_ms > 0 else None,
+            "issue_slots_per_nnz_at_measured_rate": 4 * sm_count * clk * (k_ms * 1e-3) / nnz if nnz else None,
+            "dram_GBs_ncu": traffic_bytes / (k_ms * 1e-3) / 1e9 if traffic_bytes and k_ms > 0 else None,
+            "sm_count": sm_count, "sm_mhz": sm_mhz,
+            "model": "one 128 B L1 wavefront/clk/SM; row from L2 = 1.5 pipe cycles, record = 0.5 (DESIGN.md Sec. 6); "
+                     "l1_lines_gnnz_s = the rate at which >= 1 row per nonzero can pass the pipe at all; "
+                     "issue slots = 4 schedulers x SMs x clock x launch time / nnz"}
 
 
 def extra_rows(P, W, args, dev, peak, skip_config):
@@ -438,15 +486,25 @@ def run_ours(args):
     peak, peak_src = hbm_peak()
     k_ms, alg_bytes_launch, achieved, breakdown = case.kernel_classes(args.steps)
     prof = ncu_traffic(args.config, R) if not args.nnz else None
+    sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+    sm_mhz = float(clocks.get("sm_mhz") or 1965.0) if isinstance(clocks, dict) else 1965.0
+    rows_per_nnz = case.rows_gathered_per_nnz() if nnz else [0.0] * N
+    traffic = prof["traffic"] if prof else None
+    # Two fractions, kept apart: `frac` / `algorithmic_frac` = compulsory bytes over time (the contract's figure);
+    # `dram_frac` = what the DRAM actually moved (ncu dram bytes of the committed capture) over THIS run's launch time.
     roofline = {"bound": "hbm", "kernel": "k_mttkrp", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": prof["traffic"] if prof else None, "peak_source": peak_src,
+                "frac": achieved / peak, "algorithmic_frac": achieved / peak,
+                "dram_frac": (traffic / (k_ms * 1e-3) / 1e9 / peak) if traffic and k_ms > 0 else None,
+                "traffic": traffic, "peak_source": peak_src,
+                "ceilings": pipe_ceilings(rows_per_nnz, nnz, R, k_ms, sm_count, sm_mhz, traffic) if nnz else None,
                 "traffic_source": (prof["source"] + " (ncu --set full capture of the committed build; a profile constant, "
                                    "not measured by this run)") if prof else None,
                 "l2_hit_pct_ncu": prof["l2_hit_pct"] if prof else None, "l1_hit_pct_ncu": prof["l1_hit_pct"] if prof else None,
                 "frac_of_nominal_8TBs": achieved / 8000.0,
                 "algorithmic_bytes_per_launch": alg_bytes_launch, "avg_launch_ms": k_ms,
                 "per_mode_algorithmic_bytes": case.bytes_mode,
-                "binding_limit": "L1 data pipe: one 128-byte wavefront per clock per SM, >= 1 per nonzero (DESIGN.md Sec. 6)"}
+                "binding_limit": "nominal bound HBM; the nearer ceiling is the L1 data pipe (`ceilings`), and the kernel is "
+                                 "latency-bound below both: gathered rows in flight per SM (DESIGN.md Sec. 6)"}
 
     # end to end through the host-buffer entry point (H2D of all factors + D2H of all Y_d every step)
     e2e = None
@@ -489,6 +547,8 @@ def run_ours(args):
                "remap_create_time_ms": {"plain": [round(x, 3) for x in info["remap_plain_ms"]],
                                         "two_pass": [round(x, 3) for x in info["remap_twopass_ms"]]},
                "bytes_held": info["bytes_held"], "bytes_paper_format": info["bytes_paper_format"],
+               "bytes_held_per_nnz": info["bytes_held"] / max(nnz, 1),
+               "bytes_paper_format_per_nnz": info["bytes_paper_format"] / max(nnz, 1),
                "create_s": case.create_s, "generate_s": case.generate_s}
     launches = case.launches_per_sweep * args.steps
     case.close()

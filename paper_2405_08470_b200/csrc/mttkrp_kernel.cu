@@ -412,7 +412,7 @@ __device__ __forceinline__ void shard_body(const KernelArgs<N>& a, const int64_t
             float val[B];
             bool e1[B];
             uint32_t anyend = 0;                              // OR of the batch's word 0: sign set = some output row ends in it
-            auto P = [&](uint32_t base) {                     // `base` = ring byte address of the batch's first record
+            auto batch_prefetch = [&](uint32_t base) {                     // `base` = ring byte address of the batch's first record
                 uint4 q[B];
 #pragma unroll
                 for (int s = 0; s < B; ++s) q[s] = lds128(base + 4u * (uint32_t)(s * ROWW));
@@ -432,7 +432,7 @@ __device__ __forceinline__ void shard_body(const KernelArgs<N>& a, const int64_t
                     anyend |= q[s].x;
                 }
             };
-            auto C = [&](uint32_t base) {
+            auto batch_compute = [&](uint32_t base) {
                 if (!__any_sync(0xffffffffu, (int32_t)anyend < 0)) {      // common: no output row ends in this batch
 #pragma unroll
                     for (int s = 0; s < B; ++s) {
@@ -457,7 +457,7 @@ __device__ __forceinline__ void shard_body(const KernelArgs<N>& a, const int64_t
             for (int r = 0; r < AHEAD; ++r) issue_round();
             cp_async_wait<AHEAD - 1>();                       // round 0 has landed
             __syncwarp();
-            P(ring_gs);
+            batch_prefetch(ring_gs);
             int stage = 0;
             for (int r = 0; r < nrounds; ++r) {
                 issue_round();                                // round r+AHEAD, reuses the stage of round r-1
@@ -494,9 +494,9 @@ __device__ __forceinline__ void shard_body(const KernelArgs<N>& a, const int64_t
 #endif
 #pragma unroll
                 for (int b = 0; b < K / B; ++b) {
-                    C(cs + 4u * (uint32_t)(b * B * ROWW));
-                    if (b + 1 < K / B) P(cs + 4u * (uint32_t)((b + 1) * B * ROWW));
-                    else if (r + 1 < nrounds) P(ns);
+                    batch_compute(cs + 4u * (uint32_t)(b * B * ROWW));
+                    if (b + 1 < K / B) batch_prefetch(cs + 4u * (uint32_t)((b + 1) * B * ROWW));
+                    else if (r + 1 < nrounds) batch_prefetch(ns);
                 }
                 stage = nstage;
                 __syncwarp();                                 // everyone is done with round r's stage
