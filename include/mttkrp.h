@@ -87,7 +87,12 @@ typedef struct {
     int64_t num_shards;                  /* ceil(nnz / shard_nnz); same for every mode */
     int64_t num_split_rows[MTTKRP_MAX_MODES];  /* output rows whose nonzeros span more than one shard */
     int64_t num_empty_rows[MTTKRP_MAX_MODES];  /* output rows with no nonzero (stored as zeros) */
-    int64_t bytes_held;                  /* device bytes the handle keeps after create (both tensor copies, maps, tables) */
+    int64_t bytes_held;                  /* device bytes the handle keeps after create (both tensor copies, maps, tables,
+                                            staging for the *_host entry points): the handle uses workspace[0, bytes_held)
+                                            and never touches the bytes from bytes_held on once mttkrp_create has returned,
+                                            so the caller may reuse them.  It is below mttkrp_workspace_bytes by the
+                                            create-time scratch and by the walk maps (8 bytes per nonzero) of every
+                                            remap transition whose measured walk turned out to be the plain one */
     int64_t bytes_paper_format;          /* FLYCOO bytes by the paper's formula, PAPER.md:187:
                                             nnz * (N*ceil(log2 nnz) + sum ceil(log2 I_h) + 32) / 8 */
     int64_t remaps_done;                 /* remap passes executed since create */

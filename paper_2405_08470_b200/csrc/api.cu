@@ -208,7 +208,7 @@ mttkrp_status_t mttkrp_create(mttkrp_handle_t* out, int nmodes, const int64_t* d
             h->stage_out[d] = reinterpret_cast<float*>(ws + p.stage_out[d]);
         }
     }
-    h->bytes_held = (int64_t)(p.persistent_end + (size_t)lp.rec_words * 4 * (size_t)(p.num_shards * p.shard_nnz));
+    h->bytes_held = (int64_t)p.total;                             // until build_format has chosen the walks
     mttkrp_status_t s = build_format(h, p, ws, idx, vals, static_cast<cudaStream_t>(cuda_stream));
     if (s != MTTKRP_OK) { cudaEventDestroy(h->ev_order); delete h->timing; delete h; return s; }
     order_end(h, static_cast<cudaStream_t>(cuda_stream));

@@ -58,8 +58,6 @@ mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_
     size_t off = 0;
     p->rec_a = off; off = align_up(off + rec_bytes);
     for (int d = 0; d < N; ++d) { p->next[d] = off; off = align_up(off + 4 * n); }
-    for (int d = 0; d < N; ++d) { p->ord[d] = off; off = align_up(off + 4 * n); }
-    for (int d = 0; d < N; ++d) { p->osrc[d] = off; off = align_up(off + 4 * n); }
     for (int d = 0; d < N; ++d) { p->lflags[d] = off; off = align_up(off + (size_t)(p->num_shards * p->shard_nnz)); }
     p->perm0 = off; off = align_up(off + 4 * n);
     // composed maps for out-of-order calls: a jump of k layouts composes k-1 times (ping-pong when k > 2)
@@ -89,7 +87,17 @@ mttkrp_status_t plan_workspace(int N, const int64_t* dims, int64_t nnz, int max_
     scratch += 4096;                                                  // counters, error flag
     for (int d = 0; d < N; ++d) scratch += align_up(4 * ((size_t)dims[d] + 1));   // index degrees (cold-row marks)
     scratch += align_up(4 * kDegBins);                                // degree histogram
-    p->total = off + std::max(align_up(rec_bytes), scratch);
+    // ord / osrc (8 bytes per nonzero per transition) sit in a pool at the very END of the workspace: which
+    // transitions need them is only known once create has measured the walks, and those that do are then moved to the
+    // front of the pool (build_format), so that everything the handle still uses afterwards is one prefix of the
+    // workspace (info.bytes_held) and the rest is the caller's again.
+    p->pool = off + std::max(align_up(rec_bytes), scratch);
+    p->pool_slot = align_up(4 * n);
+    for (int d = 0; d < N; ++d) {
+        p->ord[d] = p->pool + (size_t)(2 * d) * p->pool_slot;
+        p->osrc[d] = p->pool + (size_t)(2 * d + 1) * p->pool_slot;
+    }
+    p->total = p->pool + (size_t)(2 * N) * p->pool_slot;
     return MTTKRP_OK;
 }
 
@@ -967,6 +975,28 @@ mttkrp_status_t build_format(mttkrp_handle_s* h, const WorkspacePlan& plan, char
         }
         h->remaps_done = 0;                                      // the tensor is back in the mode-0 layout (N transitions per cycle)
     }
+    // Give back what the chosen walks do not need: the slot pairs of the transitions that read ord / osrc move to the
+    // front of the pool (lower addresses only, in mode order, on the stream: a destination slot was vacated or never
+    // used), the other modes lose their pointers, and the handle holds the workspace up to the last used slot.
+    int used = 0;
+    for (int d = 0; d < N; ++d) {
+        ModeMeta& mm = h->mode[d];
+        if (nnz > 0 && mm.blocked != 0) {
+            uint32_t* o = reinterpret_cast<uint32_t*>(ws + plan.pool + (size_t)(2 * used) * plan.pool_slot);
+            uint32_t* s2 = reinterpret_cast<uint32_t*>(ws + plan.pool + (size_t)(2 * used + 1) * plan.pool_slot);
+            if (o != mm.ord) {
+                MK_CUDA(cudaMemcpyAsync(o, mm.ord, 4 * n, cudaMemcpyDeviceToDevice, st));
+                MK_CUDA(cudaMemcpyAsync(s2, mm.osrc, 4 * n, cudaMemcpyDeviceToDevice, st));
+            }
+            mm.ord = o;
+            mm.osrc = s2;
+            ++used;
+        } else {
+            mm.ord = mm.osrc = nullptr;
+        }
+    }
+    const size_t rec_bytes = (size_t)h->rec_words * 4 * (size_t)(nshards * S);
+    h->bytes_held = (int64_t)(used ? plan.pool + (size_t)(2 * used) * plan.pool_slot : plan.persistent_end + rec_bytes);
     return MTTKRP_OK;
 }
 

@@ -129,7 +129,8 @@ struct ModeMeta {
     PackDesc pk;              // bit layout of this layout's packed records (handle->packed)
     uint32_t* next;           // [nnz] gather map of the remap d -> (d+1)%N: position in THIS layout of the
                               // element at position j of the next layout (the paper's remap id, read backwards)
-    uint32_t* ord;            // [nnz] positions of the NEXT layout ordered by the 2^block_log2-record block of this
+    uint32_t* ord;            // (NULL after create when the chosen walk is the plain one)
+                              // [nnz] positions of the NEXT layout ordered by the 2^block_log2-record block of this
                               // layout they come from (stable), or unused: the blocked remap walks the destination
                               // in this order so that its random reads stay inside one L2-resident window at a time
     uint32_t* osrc;           // [nnz] osrc[t] = next[ord[t]]: the source position of walk step t (saves the walk one
@@ -227,6 +228,7 @@ struct WorkspacePlan {
     size_t stage_fac[kMaxModes], stage_out[kMaxModes];
     size_t persistent_end;
     size_t scratch;          // start of the create-time scratch (may overlap rec_b)
+    size_t pool, pool_slot;  // ord / osrc pool at the end of the workspace: 2*N slots of pool_slot bytes (ord[d], osrc[d])
     size_t total;
     int shard_nnz;
     int64_t num_shards;

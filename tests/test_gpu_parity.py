@@ -280,6 +280,25 @@ def test_record_formats_for_four_and_more_modes(P, monkeypatch, pack):
         assert info["record_bytes"] == (16 if pack == "1" else 4 * (N + 1))
 
 
+@pytest.mark.parametrize("pack", ["0", "1"])
+@pytest.mark.parametrize("dims,cid", [((400_000, 30, 17, 2500, 9, 12), 96), ((300_000, 6, 5, 700, 4, 3, 40, 2), 98)])
+def test_mid_size_six_and_eight_modes_all_entries(P, monkeypatch, dims, cid, pack):
+    # More than 4 modes is one of the paper's claims (Sec. 5.6), and the N = 6..8 instantiations have
+    # their own occupancy targets and > 48 KB shared-memory geometry.  A million nonzeros gives them what the tiny
+    # tensors cannot: hundreds of shards (a multi-wave grid), rows split across many shards (the 2..40-row modes),
+    # empty rows (the Zipf mode), both record formats, the narrowest and the widest rank - every entry of every Y_d and
+    # every permutation against the oracle.
+    monkeypatch.setenv("MTTKRP_PACK", pack)
+    N = len(dims)
+    spec = W.TensorSpec(f"mid{N}", list(dims), 1_000_003, [1.2] + [0.0] * (N - 1), "uniform", (8, 64), cid)
+    t = W.generate_tensor(spec)
+    for R in (8, 64):
+        worst, info = _run_case(P, list(dims), t.idx, t.vals, R, seed=cid + R, check_perm=(R == 8))
+        assert info["record_bytes"] == (16 if pack == "1" else 4 * (N + 1))
+        assert info["num_shards"] >= 100
+        assert max(info["num_split_rows"]) > 0 and info["num_empty_rows"][0] > 0
+
+
 def test_wide_index_tensor_falls_back_to_unpacked_records(P):
     # 3 x 22 bits of leading keys do not fit the 64-bit key string: the handle keeps 20-byte records.
     # (The cell count exceeds 64 bits, so the COO list is drawn directly; duplicates are legal and add.)
@@ -313,6 +332,57 @@ def test_blocked_walk_is_chosen_from_measured_runs(P):
     info = h.info()
     assert info["remap_blocked"] == [1, 1, 1] and min(info["remap_avg_run"]) >= 4
     h.destroy()
+
+
+@pytest.mark.parametrize("walk", ["measured", "twopass", "blocked"])
+def test_workspace_beyond_bytes_held_is_the_callers(P, monkeypatch, walk):
+    # info.bytes_held is a promise: after create the handle lives in workspace[0, bytes_held) - the walk maps of
+    # transitions that ended up with the plain walk, and the create-time scratch, are given back.  Overwrite
+    # everything from bytes_held on and every call must still match the oracle (permutation, remapped copy, Y).
+    if walk == "twopass":
+        monkeypatch.setenv("MTTKRP_REMAP_TWOPASS", "1")
+        monkeypatch.setenv("MTTKRP_TWOPASS_WINDOW_LOG2", "11")
+    if walk == "blocked":
+        monkeypatch.setenv("MTTKRP_REMAP_BLOCKED", "1")
+        monkeypatch.setenv("MTTKRP_REMAP_BLOCK_LOG2", "12")
+    dev = torch.device("cuda:0")
+    for cfg, nnz, R in [(0, 100_000, 16), (2, 260_003, 32), (3, 90_007, 8)]:
+        spec = W.CONFIGS[cfg].scaled(nnz)
+        t = W.generate_tensor(spec)
+        dims, N = list(spec.dims), len(spec.dims)
+        h = P.Mttkrp(dims, t.idx.to(dev), t.vals.to(dev))
+        info = h.info()
+        total = P.mttkrp_workspace_bytes(dims, t.nnz)
+        held = info["bytes_held"]
+        slot = -(-4 * t.nnz // 256) * 256                               # one walk map, 256-byte aligned
+        users = sum(1 for w in info["remap_blocked"] if w != 0)
+        assert 0 < held <= total
+        if users == 0:
+            assert held <= total - 2 * N * slot                         # plain walks everywhere: the whole pool is free
+        else:
+            assert held == total - 2 * (N - users) * slot
+        if walk == "measured":
+            assert users == 0                                           # too small for the blocked / two-pass walks
+        else:
+            assert users > 0
+        off = h._ws_ptr - h.workspace.data_ptr()
+        h.workspace[off + held:].fill_(0xA5)
+        idx_np, vals_np = t.idx.numpy(), t.vals.numpy()
+        fac_np = [np.random.default_rng(40 + m).uniform(-1, 1, size=(d, R)).astype(np.float32) for m, d in enumerate(dims)]
+        fac = [torch.from_numpy(f).to(dev) for f in fac_np]
+        for d in list(range(N)) + [0, N - 1, 1, 0]:                     # cyclic sweep, then out-of-order jumps
+            perm = oracle.sort_perm(dims, idx_np, info["key_order"][d])
+            out = torch.full((dims[d], R), float("nan"), dtype=torch.float32, device=dev)
+            Y = h.mttkrp_mode(d, fac, out=out).cpu().numpy()
+            gi, gv = h.export_coo()
+            np.testing.assert_array_equal(gi.cpu().numpy(), idx_np[:, perm])
+            np.testing.assert_array_equal(gv.cpu().numpy(), vals_np[perm])
+            np.testing.assert_array_equal(h.get_perm(d).cpu().numpy().astype(np.int64), perm)
+            Yo, So = oracle.mttkrp_mode(dims, idx_np, vals_np, fac_np, d, perm=perm)
+            err, zeros_ok = oracle.normalised_error(Y, Yo, So)
+            assert zeros_ok and err <= TOL
+        assert bool((h.workspace[off + held:] == 0xA5).all()), "the handle wrote beyond bytes_held"
+        h.destroy()
 
 
 def _sample_rows(idx_d, dim, rng, k=48):
