@@ -75,10 +75,9 @@ __device__ __forceinline__ Vec vzero() {
     return r;
 }
 
-#ifndef MK_L2HINT        // 1: the record stream is read with an L2 evict-first policy, so that it does not push the
-#define MK_L2HINT 1      //    factor rows (the data that is re-used) out of L2 (measured: -2 % on configs[1], -1 % on
-                         //    configs[2]; an evict-last hint on the factor rows themselves was 10 % slower)
-#endif
+// The record stream is read with an L2 evict-first policy, so that it does not push the factor rows (the data that is
+// re-used) out of L2 (measured: -2 % on configs[1], -1 % on configs[2]; an evict-last hint on the factor rows
+// themselves was 10 % slower).
 __device__ __forceinline__ uint64_t l2_policy_evict_first() {
     uint64_t p;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
@@ -87,48 +86,11 @@ __device__ __forceinline__ uint64_t l2_policy_evict_first() {
 // One lane's 4 columns of a factor row (read-only path, 128-bit load).  `base` = this lane's slot in row 0 of
 // the factor matrix (float4 units), `key` = row index, LPN = lanes per row: the address is one 32x32->64
 // multiply-add on a per-lane base.  Needs dims[m] < 2^28 (api.cu check_shape).
-#ifndef MK_ROWPOL        // experiment: L2 eviction policy of the factor-row gathers. 0 = default; 1 = evict_last with fraction
-#define MK_ROWPOL 0      // MK_ROWPOL_FRAC on all rows; 2 = on fiber-level rows only; 3 = evict_first on last-level rows only
-#endif
-#ifndef MK_ROWPOL_FRAC
-#define MK_ROWPOL_FRAC 0.5
-#endif
-#define MK_STR2(x) #x
-#define MK_STR(x) MK_STR2(x)
-#ifndef MK_L1POL         // experiment: L1 eviction priority per LEVEL (uniform per instruction). 1: last level no_allocate;
-#define MK_L1POL 0       // 2: last level evict_first; 3: fiber level evict_last; 4: fiber evict_last + last evict_first;
-#endif                   // 5: fiber evict_last + last no_allocate
-__device__ __forceinline__ float4 ldg_pol(const float4* p, int kind) {   // kind 0: last level, 1: fiber level
-#if MK_ROWPOL == 0 && MK_L1POL == 0
-    (void)kind;
-    return __ldg(p);
-#elif MK_ROWPOL == 0
-    float4 v;
-    if (kind == 0 && (MK_L1POL == 1 || MK_L1POL == 5))
-        asm("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
-    else if (kind == 0 && (MK_L1POL == 2 || MK_L1POL == 4))
-        asm("ld.global.nc.L1::evict_first.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
-    else if (kind == 1 && MK_L1POL >= 3)
-        asm("ld.global.nc.L1::evict_last.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
-    else v = __ldg(p);
-    return v;
-#else
-    float4 v;
-    const bool last_pol = (MK_ROWPOL == 1 || MK_ROWPOL == 3), fiber_pol = (MK_ROWPOL == 1 || MK_ROWPOL == 2);
-    if ((kind == 0 && last_pol) || (kind == 1 && fiber_pol)) {
-        uint64_t pol;
-        if (MK_ROWPOL == 3) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-        else asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, " MK_STR(MK_ROWPOL_FRAC) ";" : "=l"(pol));
-        asm volatile("ld.global.nc.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p), "l"(pol));
-    } else {
-        v = __ldg(p);
-    }
-    return v;
-#endif
-}
+// (Per-row L2 eviction policies and per-level L1 eviction priorities on these gathers were measured in rounds 1-2 and
+// all lost to the plain read-only load; the numbers are in DESIGN.md Sec. 6, the switches are gone.)
 template <int LPN>
 __device__ __forceinline__ Vec ld_row(const float4* __restrict__ base, uint32_t key) {
-    const float4 v = ldg_pol(base + (size_t)key * LPN, 0);
+    const float4 v = __ldg(base + (size_t)key * LPN);
     Vec r;
     r.p[0] = make_float2(v.x, v.y);
     r.p[1] = make_float2(v.z, v.w);
@@ -141,7 +103,7 @@ template <int LPN>
 __device__ __forceinline__ Vec ld_row_flagged(const float* __restrict__ base, uint32_t word, uint32_t sub) {
     constexpr int SH = LPN == 16 ? 4 : (LPN == 8 ? 3 : (LPN == 4 ? 2 : 1));
     const uint32_t off = ((SH >= 2 ? word : (word & kKeyMask)) << SH) + sub;      // the shift drops bits 30 / 31 (flag, cold mark)
-    const float4 v = ldg_pol(reinterpret_cast<const float4*>(base) + off, 1);
+    const float4 v = __ldg(reinterpret_cast<const float4*>(base) + off);
     Vec r;
     r.p[0] = make_float2(v.x, v.y);
     r.p[1] = make_float2(v.z, v.w);
@@ -162,12 +124,7 @@ __device__ __forceinline__ void vstore(float* dst, const Vec& v) {
 }
 
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, uint64_t policy) {
-#if MK_L2HINT
     asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "l"(policy) : "memory");
-#else
-    (void)policy;
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
-#endif
 }
 __device__ __forceinline__ void cp_async8(uint32_t dst, const void* src) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
@@ -184,14 +141,9 @@ __device__ __forceinline__ uint4 lds128(uint32_t addr) {
     return v;
 }
 // Requests the line of a factor row into L2 (SASS CCTL.E.PF2: no register, no scoreboard).
-#ifndef MK_PREFETCH      // 0: off; 1: one request per row; 2: both 64-byte halves
-#define MK_PREFETCH 1
-#endif
+// One request per row (requesting both 64-byte halves measured slower).
 __device__ __forceinline__ void prefetch_l2(const float4* row) {
     asm volatile("prefetch.global.L2 [%0];" ::"l"(row));
-#if MK_PREFETCH >= 2
-    asm volatile("prefetch.global.L2 [%0];" ::"l"(row + 4));
-#endif
 }
 __device__ __forceinline__ uint32_t lds32(uint32_t addr) {
     uint32_t v;
@@ -200,24 +152,9 @@ __device__ __forceinline__ uint32_t lds32(uint32_t addr) {
 }
 
 // ---- compile-time geometry ---------------------------------------------------------------------
-#ifndef MK_D             // gather look-ahead of the default variant, in steps
-#define MK_D 2
-#endif
-#ifndef MK_D_DEEP        // ... of the DEEP variant
-#define MK_D_DEEP 4
-#endif
-#ifndef MK_OPAQUE
-#define MK_OPAQUE 1
-#endif
-#ifndef MK_STAGES
-#define MK_STAGES 3
-#endif
-#ifndef MK_MINB          // resident blocks per SM the register allocation must allow; 0 = per-N default below.
-#define MK_MINB 0        // Measured on B200 (configs[1], configs[2]): occupancy beats deeper look-ahead.
-#endif
-#ifndef MK_MINB_DEEP
-#define MK_MINB_DEEP 0
-#endif
+constexpr int kLookAhead = 2;        // gather look-ahead of the default variant, in steps
+constexpr int kLookAheadDeep = 4;    // ... of the DEEP variant
+constexpr int kRingStages = 3;       // record ring: round r computing, r+1 landed, the rest in flight
 template <int N, int R, bool DEEP, bool PACKED>
 struct Geo {
     static constexpr int V = 4;                          // rank columns per lane
@@ -228,17 +165,18 @@ struct Geo {
     static constexpr int RECW = PACKED ? 4 : N + 1;      // record words
     static constexpr int SLOTW = (RECW + 3) / 4 * 4;     // ring slot words (16-byte multiple)
     static constexpr int K = (NPW * SLOTW <= 32) ? 8 : 4;  // records per group per ring stage
-    static constexpr int STAGES = MK_STAGES;             // round r computing, r+1 landed, the rest in flight
+    static constexpr int STAGES = kRingStages;           // round r computing, r+1 landed, the rest in flight
     // gather look-ahead, in steps (K % D == 0).  DEEP: twice the look-ahead at fewer blocks per SM, for
     // factor matrices that do not fit L2 (every gather that misses is a random HBM access).
-    static constexpr int D0 = (DEEP && N <= 3) ? MK_D_DEEP : MK_D;
+    static constexpr int D0 = (DEEP && N <= 3) ? kLookAheadDeep : kLookAhead;
     static constexpr int D = (D0 < K) ? D0 : K / 2;
     static constexpr int RING_WORDS = STAGES * K * NPW * SLOTW;        // per warp
     static constexpr int ENT_WORDS = 2 * NPW * R;                       // per warp: first/last partial rows
     static constexpr int WARP_WORDS = RING_WORDS > ENT_WORDS ? RING_WORDS : ENT_WORDS;
     static constexpr int NL = N - 1;                     // accumulator levels t[0..NL-1]
-    static constexpr int MINB_DEF = N <= 3 ? (DEEP ? 3 : 5) : (N == 4 ? (PACKED ? 4 : 3) : (N == 5 ? 3 : 2));   // no instantiation spills
-    static constexpr int MINB = DEEP ? (MK_MINB_DEEP ? MK_MINB_DEEP : MINB_DEF) : (MK_MINB ? MK_MINB : MINB_DEF);
+    // resident blocks per SM the register allocation must allow: no instantiation spills, and on B200 (configs[1],
+    // configs[2]) occupancy beat deeper look-ahead
+    static constexpr int MINB = N <= 3 ? (DEEP ? 3 : 5) : (N == 4 ? (PACKED ? 4 : 3) : (N == 5 ? 3 : 2));
     static constexpr int SMEM_BYTES = 4 * (WARPS * WARP_WORDS + WARPS * NPW * R + 2 * WARPS * R + WARPS * 2 * NPW + 2 * WARPS);
 };
 
@@ -319,22 +257,13 @@ __device__ __forceinline__ void shard_body(const KernelArgs<N>& a, const int64_t
     uint32_t* const ring = &s_warp[warp][0];
     const uint32_t* const ring_g = ring + g * SLOTW;      // this group's column of the ring
     uint32_t ring_gs = (uint32_t)__cvta_generic_to_shared(ring_g);
-#if MK_OPAQUE
     asm volatile("mov.u32 %0, %0;" : "+r"(ring_gs));     // opaque: kept in a register instead of being re-derived from %tid every round
-#endif
 
     // per-lane bases of the factor rows: row r of level l = fb[l] + r * LPN (float4 units)
     const float4* fb[N];
 #pragma unroll
     for (int l = 1; l < N; ++l) fb[l] = reinterpret_cast<const float4*>(a.fac[l]) + sub;
-#if MK_OPAQUE >= 2
-    // Register-resident base of the deepest fiber level: without it every fiber-row gather reloads the pointer
-    // from the constant bank (LDC), which costs an issue slot and, worse, one of the six scoreboards.
     const float* fiber_base = NL >= 2 ? a.fac[NL >= 2 ? NL - 1 : 1] : nullptr;
-    if constexpr (NL >= 2) asm volatile("mov.u64 %0, %0;" : "+l"(fiber_base));
-#else
-    const float* fiber_base = NL >= 2 ? a.fac[NL >= 2 ? NL - 1 : 1] : nullptr;
-#endif
 
     // ---- record ring fill ---------------------------------------------------------------------------------
     const uint64_t rec_policy = l2_policy_evict_first();
@@ -342,9 +271,7 @@ __device__ __forceinline__ void shard_body(const KernelArgs<N>& a, const int64_t
     // pointer just advances by one round per call.
     const uint32_t* fill_src = grec + (size_t)sub * RECW;
     uint32_t fill_dst = ring_gs + 4u * (uint32_t)(sub * ROWW);           // ring slot of record `sub` in stage 0
-#if MK_OPAQUE
     asm volatile("mov.u32 %0, %0;" : "+r"(fill_dst));
-#endif
     int fill_round = 0, fill_stage = 0;
     auto issue_round = [&]() {
         if (fill_round < nrounds) {
@@ -403,10 +330,7 @@ __device__ __forceinline__ void shard_body(const KernelArgs<N>& a, const int64_t
             // steps are read with back-to-back LDS.128, their B last-level rows and up to B fiber rows are requested
             // together (up to 8 independent 128-bit gathers per lane in flight), then the B steps are computed.  Costs
             // 80 registers (3 blocks per SM); one vote per batch replaces the per-step output-row-end test.
-#ifndef MK_B
-#define MK_B 4
-#endif
-            constexpr int B = MK_B;
+            constexpr int B = 4;                                  // (2 and 8 measured slower on configs[2])
             static_assert(K % B == 0, "batch");
             Vec al[B], rb[B];
             float val[B];
@@ -461,22 +385,19 @@ __device__ __forceinline__ void shard_body(const KernelArgs<N>& a, const int64_t
             int stage = 0;
             for (int r = 0; r < nrounds; ++r) {
                 issue_round();                                // round r+AHEAD, reuses the stage of round r-1
-#ifndef MK_PF_DIST       // rounds between the L2 prefetch of a cold row and its gather (needs MK_STAGES >= MK_PF_DIST + 2)
-#define MK_PF_DIST 1
-#endif
-                static_assert(AHEAD >= MK_PF_DIST, "prefetch distance");
-                cp_async_wait<AHEAD - MK_PF_DIST>();          // rounds <= r+MK_PF_DIST have landed
+                constexpr int PF_DIST = 1;                    // rounds between the L2 prefetch of a cold row and its gather (STAGES >= PF_DIST + 2)
+                static_assert(AHEAD >= PF_DIST, "prefetch distance");
+                cp_async_wait<AHEAD - PF_DIST>();             // rounds <= r+PF_DIST have landed
                 __syncwarp();
                 const int nstage = (stage + 1 == STAGES) ? 0 : stage + 1;
                 const uint32_t cs = ring_gs + 4u * (uint32_t)(stage * STAGEW);
                 const uint32_t ns = ring_gs + 4u * (uint32_t)(nstage * STAGEW);
-                const uint32_t ps = ring_gs + 4u * (uint32_t)(((stage + MK_PF_DIST) % STAGES) * STAGEW);
-#if MK_PREFETCH
+                const uint32_t ps = ring_gs + 4u * (uint32_t)(((stage + PF_DIST) % STAGES) * STAGEW);
                 // Cold rows (common.cuh: outside the K most frequent of their factor matrix, so they almost always miss
                 // L2 when the factors overflow it) of the NEXT round are requested into L2 now, one round (~3000 clk)
                 // before their gathers; lane p of the group looks at record p of that round.  The batch then waits for
                 // L2 hits instead of HBM reads (configs[2]: -7 % per mode).
-                if (r + MK_PF_DIST < nrounds) {
+                if (r + PF_DIST < nrounds) {
 #pragma unroll
                     for (int i = 0; i < (K + LPN - 1) / LPN; ++i) {
                         const int pr = sub + i * LPN;
@@ -491,7 +412,6 @@ __device__ __forceinline__ void shard_body(const KernelArgs<N>& a, const int64_t
                         }
                     }
                 }
-#endif
 #pragma unroll
                 for (int b = 0; b < K / B; ++b) {
                     batch_compute(cs + 4u * (uint32_t)(b * B * ROWW));
@@ -902,9 +822,6 @@ static mttkrp_status_t launch_nr(mttkrp_handle_s* h, int d, const float* const* 
             constexpr int smem = Geo<N, R, DEEP, PACKED>::SMEM_BYTES;
             if constexpr (smem > 48 * 1024)               // per device, so not cached in a static
                 MK_CUDA(cudaFuncSetAttribute(k_mttkrp<N, R, DEEP, PACKED>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-#ifdef MK_CARVEOUT                                          // experiment: shared-memory carveout in percent of the maximum
-            MK_CUDA(cudaFuncSetAttribute(k_mttkrp<N, R, DEEP, PACKED>, cudaFuncAttributePreferredSharedMemoryCarveout, MK_CARVEOUT));
-#endif
             TimedLaunch tl(h->timing, kClsMttkrp, st);
             k_mttkrp<N, R, DEEP, PACKED><<<(unsigned)h->num_shards, kBlockThreads, smem, st>>>(a);
             return MTTKRP_OK;
