@@ -30,7 +30,7 @@ if ROOT not in sys.path:
 METRIC = "all-mode spMTTKRP GFLOP/s (nnz*N*R flops per mode, remap included)"
 UNIT = "GFLOP/s"
 FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback
-TRAFFIC_CSV = os.path.join("profiles", "r2_traffic.csv")   # ncu dram bytes per launch of the committed build
+TRAFFIC_CSV = os.path.join("profiles", "r3_traffic.csv")   # ncu dram bytes per launch of the committed build
 
 
 def parse_args():
@@ -157,6 +157,29 @@ def oracle_pass(dims, idx, vals, fac, R, perms=None):
     return t_acc, t_sort, out_perms
 
 
+def one_thread_small_case():
+    """the oracle on ONE thread, the literal definition, on configs[0] (100k nonzeros, R = 16):
+    sort + accumulation for all modes, wall clock, best of 3."""
+    import oracle
+    import workloads as W
+    spec = W.CONFIGS[0]
+    R = default_rank(spec)
+    t = W.generate_tensor(spec)
+    idx, vals = t.idx.numpy(), t.vals.numpy()
+    fac = [f.numpy() for f in W.generate_factors(spec, R)]
+    N = len(spec.dims)
+    best = None
+    for _ in range(3):
+        t0 = time.perf_counter()
+        for d in range(N):
+            perm = oracle.sort_perm(spec.dims, idx, [d])
+            oracle.mttkrp_mode(spec.dims, idx, vals, fac, d, perm=perm, threads=1)
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+    return {"workload": workload_name(spec, R), "threads": 1, "seconds": best, "value": float(t.nnz) * N * R * N / best / 1e9,
+            "unit": UNIT, "what": "stable sort + fp64 accumulation, all modes, best of 3"}
+
+
 def cpu_baseline_leg(spec, R, idx, vals, fac_np, sample_nnz):
     import numpy as np
     import oracle
@@ -173,6 +196,7 @@ def cpu_baseline_leg(spec, R, idx, vals, fac_np, sample_nnz):
     t_acc, t_sort, _ = oracle_pass(spec.dims, idx, vals, fac_np, R)
     flops = float(n) * N * R * N
     return {"value": flops / t_acc / 1e9, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
+            "one_thread_configs0": one_thread_small_case(),
             "sample": f"{what}, all {N} modes, fp64 oracle as it stands (not a tuned CPU implementation): accumulation "
                       f"{t_acc:.2f} s on all cores; its one-thread stable sort ({t_sort:.2f} s) is its format build and, "
                       f"like mttkrp_create on the GPU side, is not in the figure",
@@ -232,7 +256,7 @@ def hbm_peak():
 
 
 def ncu_traffic(config_id, R):
-    """dram bytes per k_mttkrp launch from the committed ncu capture of this build (profiles/r2_traffic.csv);
+    """dram bytes per k_mttkrp launch from the committed ncu capture of this build (profiles/r3_traffic.csv);
     a constant of the committed profile, not measured by this run - None when no capture matches."""
     path = os.path.join(ROOT, TRAFFIC_CSV)
     if not os.path.exists(path):
@@ -397,7 +421,13 @@ def extra_rows(P, W, args, dev, peak, skip_config):
                          "unit": UNIT, "ms_per_step": ms / steps, "steps": steps,
                          "mttkrp_avg_launch_ms": k_ms, "mttkrp_algorithmic_GBs": achieved, "mttkrp_frac": achieved / peak,
                          "remap_ms_per_sweep": brk["remap_ms_per_sweep"], "remap_share": brk["remap_share"],
-                         "create_s": case.create_s})
+                         "create_s": case.create_s, "remap_walk": case.info["remap_blocked"],
+                         "bytes_held_per_nnz": case.info["bytes_held"] / max(case.nnz, 1)})
+            prof = ncu_traffic(c, R)                                  # profile constants of the committed capture, if any
+            if prof:
+                rows[-1].update({"traffic": prof["traffic"], "l2_hit_pct_ncu": prof["l2_hit_pct"],
+                                 "l1_hit_pct_ncu": prof["l1_hit_pct"],
+                                 "dram_frac": prof["traffic"] / (k_ms * 1e-3) / 1e9 / peak if k_ms > 0 else None})
         case.close()
     return rows
 

@@ -385,6 +385,43 @@ def test_workspace_beyond_bytes_held_is_the_callers(P, monkeypatch, walk):
         h.destroy()
 
 
+@pytest.mark.parametrize("variant", ["default", "deep", "unpacked", "twopass", "blocked", "fused", "alg1"])
+def test_repeated_sweeps_are_bit_identical(P, monkeypatch, variant):
+    # compute-sanitizer is closed on the GPU pool this library is developed on (profiles/r3_sanitizer_summary.md), so
+    # racecheck cannot vouch for the shared-memory protocol of k_mttkrp (record ring aliased with the groups' partial
+    # rows, __syncwarp hand-offs) or of k_scatter16 (shared atomics + one-warp scan).  What can be checked without
+    # it: every reduction in the path has a FIXED order, so a sweep must reproduce itself bit for bit; a hazard between
+    # warps or lanes shows up as a run-to-run difference in some entry or some record.  12 sweeps per tensor, every
+    # kernel variant, outputs and the resident copy compared with the first sweep's (which _run_case-style tests
+    # elsewhere compare with the oracle), NaN-poisoned outputs each time.
+    env = {"deep": {"MTTKRP_FORCE_DEEP": "1"}, "unpacked": {"MTTKRP_PACK": "0"},
+           "twopass": {"MTTKRP_REMAP_TWOPASS": "1", "MTTKRP_TWOPASS_WINDOW_LOG2": "11"},
+           "blocked": {"MTTKRP_REMAP_BLOCKED": "1", "MTTKRP_REMAP_BLOCK_LOG2": "12"},
+           "fused": {"MTTKRP_FUSE": "1"}, "alg1": {"MTTKRP_SHARD_POLICY": "alg1", "MTTKRP_KAPPA": "37"}}.get(variant, {})
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    dev = torch.device("cuda:0")
+    for cfg, nnz, R in [(1, 400_009, 32), (2, 300_011, 64), (3, 250_007, 32), (4, 200_003, 16)]:
+        spec = W.CONFIGS[cfg].scaled(nnz)
+        t = W.generate_tensor(spec)
+        N = len(spec.dims)
+        h = P.Mttkrp(spec.dims, t.idx.to(dev), t.vals.to(dev))
+        fac = [f.to(dev) for f in W.generate_factors(spec, R)]
+        ref, ref_coo = None, None
+        for rep in range(12):
+            outs = [torch.full((d, R), float("nan"), dtype=torch.float32, device=dev) for d in spec.dims]
+            h.mttkrp_sweep(fac, outs)
+            coo = h.export_coo()                                          # layout N-1 after a sweep
+            if ref is None:
+                ref, ref_coo = outs, coo
+                assert all(bool(torch.isfinite(y).all()) for y in outs)
+                continue
+            for d in range(N):
+                assert torch.equal(outs[d], ref[d]), f"{variant} cfg{cfg} sweep {rep} mode {d} differs from sweep 0"
+            assert torch.equal(coo[0], ref_coo[0]) and torch.equal(coo[1], ref_coo[1])
+        h.destroy()
+
+
 def _sample_rows(idx_d, dim, rng, k=48):
     """Heaviest rows, rows around shard boundaries' worth of mass, and random rows."""
     counts = torch.bincount(idx_d.long(), minlength=dim)
